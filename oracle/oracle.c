@@ -1,0 +1,619 @@
+/*
+ * oracle.c — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU statement of what the arrested-Newton-flow hot path of
+ * arxiv/paper_2603_24370 (soliton_solver) computes.  It shares no code with the CUDA
+ * path under paper_2603_24370_b200/csrc and is only ever called from tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.
+ *
+ * Every function cites the passage it follows: PAPER.md:N are line numbers of
+ * /root/reference/PAPER.md; "DESIGN R<n>" are the readings listed in DESIGN.md
+ * for the points where the paper is silent.
+ *
+ * Lattice (DESIGN R4): Nx x Ny sites INCLUDING a frozen halo of
+ * width 2; site (i,j), i fastest.  Arrays are [C][Ny][Nx] doubles.
+ * Interior I = {2<=i<Nx-2, 2<=j<Ny-2}.
+ *
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/__init__.py).
+ * -ffp-contract=off so that every expression below is evaluated exactly as written.
+ *
+ * Pins (tests/test_oracle_*.py, all "-m not gpu"):
+ *   stencils        polynomial exactness + plane-wave symbols
+ *   cm/ah energies  bond form == site form; vacuum == 0; helix / vortex closed forms
+ *   cm/ah gradients brute-force central differences of the bond-form energy (8x8)
+ *   charges         integer degree of seeded ansaetze; unit flux of a vortex
+ *   flow            RK4 order on AH; |n|=1, v.n=0; arrest invariants; Bogomolny bound
+ *   parity unpinned: the placement of the projections inside the RK4 stages
+ *   (DESIGN R7) has no external pin beyond those order/invariant checks.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define PI 3.14159265358979323846
+
+enum { ORC_CM = 0, ORC_AH = 1 };
+
+static inline size_t at(int Nx, int Ny, int c, int j, int i) {
+  return ((size_t)c * Ny + j) * Nx + i;
+}
+static inline int interior(int Nx, int Ny, int i, int j) {
+  return i >= 2 && i < Nx - 2 && j >= 2 && j < Ny - 2;
+}
+static inline int inside(int Nx, int Ny, int i, int j) {
+  return i >= 0 && i < Nx && j >= 0 && j < Ny;
+}
+
+/* ------------------------------------------------------------------ stencils */
+
+/* PAPER.md:104 eq. (1): 4th-order central first derivative, written as printed. */
+static inline double d1(double fm2, double fm1, double fp1, double fp2, double h) {
+  return (-fp2 + 8.0 * fp1 - 8.0 * fm1 + fm2) / (12.0 * h);
+}
+/* PAPER.md:109 eq. (2): 4th-order central second derivative, written as printed. */
+static inline double d2(double fm2, double fm1, double f0, double fp1, double fp2, double h) {
+  return (-fp2 + 16.0 * fp1 - 30.0 * f0 + 16.0 * fm1 - fm2) / (12.0 * (h * h));
+}
+static inline double Dx(const double* f, int Nx, int j, int i, double h) {
+  const double* p = f + (size_t)j * Nx + i;
+  return d1(p[-2], p[-1], p[1], p[2], h);
+}
+static inline double Dy(const double* f, int Nx, int j, int i, double h) {
+  const double* p = f + (size_t)j * Nx + i;
+  return d1(p[-2 * Nx], p[-Nx], p[Nx], p[2 * Nx], h);
+}
+static inline double Lx(const double* f, int Nx, int j, int i, double h) {
+  const double* p = f + (size_t)j * Nx + i;
+  return d2(p[-2], p[-1], p[0], p[1], p[2], h);
+}
+static inline double Ly(const double* f, int Nx, int j, int i, double h) {
+  const double* p = f + (size_t)j * Nx + i;
+  return d2(p[-2 * Nx], p[-Nx], p[0], p[Nx], p[2 * Nx], h);
+}
+/* Mixed derivative = eq. (1) in x applied to eq. (1) in y (16 corner points). */
+static inline double Dxy(const double* f, int Nx, int j, int i, double h) {
+  double r[5];
+  for (int k = -2; k <= 2; ++k) r[k + 2] = (k == 0) ? 0.0 : Dy(f, Nx, j, i + k, h);
+  return d1(r[0], r[1], r[3], r[4], h);
+}
+
+/* Exposed for the stencil pins: apply an operator on the interior of one plane.
+ * op: 0 Dx, 1 Dy, 2 Lx, 3 Ly, 4 DxDy.  Halo entries of out are set to 0. */
+void orc_stencil(int op, const double* f, double* out, int Nx, int Ny, double h) {
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      double r = 0.0;
+      if (interior(Nx, Ny, i, j)) {
+        switch (op) {
+          case 0: r = Dx(f, Nx, j, i, h); break;
+          case 1: r = Dy(f, Nx, j, i, h); break;
+          case 2: r = Lx(f, Nx, j, i, h); break;
+          case 3: r = Ly(f, Nx, j, i, h); break;
+          default: r = Dxy(f, Nx, j, i, h); break;
+        }
+      }
+      out[(size_t)j * Nx + i] = r;
+    }
+}
+
+/* --------------------------------------------------- canonical tree reduction */
+
+/* PAPER.md:158 ("parallel GPU reductions"), DESIGN R10: aligned pairwise tree over n
+ * values zero-padded to the next power of two: level by level t[m] = t[2m] + t[2m+1]. */
+double orc_tree_sum(const double* v, size_t n) {
+  size_t P = 1;
+  while (P < n) P <<= 1;
+  double* t = (double*)malloc(P * sizeof(double));
+  for (size_t m = 0; m < P; ++m) t[m] = (m < n) ? v[m] : 0.0;
+  while (P > 1) {
+    for (size_t m = 0; m < P / 2; ++m) t[m] = t[2 * m] + t[2 * m + 1];
+    P >>= 1;
+  }
+  double r = t[0];
+  free(t);
+  return r;
+}
+/* Row trees over x first, then one tree over the Ny row sums (DESIGN R10). */
+double orc_tree_sum2d(const double* v, int Nx, int Ny) {
+  double* rows = (double*)malloc((size_t)Ny * sizeof(double));
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < Ny; ++j) rows[j] = orc_tree_sum(v + (size_t)j * Nx, (size_t)Nx);
+  double r = orc_tree_sum(rows, (size_t)Ny);
+  free(rows);
+  return r;
+}
+
+/* ------------------------------------------------------------- chiral magnet */
+/* Functional (eq. (5), :327 Table 2, dimensionless form of BASELINE
+ * configs): e = 1/2 |grad n|^2 + kappa n.(curl n) + B(1-n3) + K(1-n3^2).
+ * Discrete energy (DESIGN R1,R3): a bond is a pair (i, j=i+k mu), mu in {x,y},
+ * k in {1,2}, both ends in the lattice and at least one end interior;
+ *   E_h = sum_bonds [ J_k/2 |n_i-n_j|^2 - 2 kappa h^2 c_k e_mu.(n_i x n_j) ]
+ *         + h^2 sum_I [ B(1-n3) + K(1-n3^2) ]
+ * with J_1 = 16/12, J_2 = -1/12 (eq. 2 weights) and c_1 = 8/(12h), c_2 = -1/(12h)
+ * (eq. 1 weights). */
+
+static const double Jw[3] = {0.0, 16.0 / 12.0, -1.0 / 12.0};
+static inline double cw(int k, double h) { /* eq. (1) weight of f(+k), k = 1,2 */
+  return (k == 1 ? 8.0 : -1.0) / (12.0 * h);
+}
+
+/* Plain definition: loop over bonds, straight summation. */
+double orc_cm_energy_bond(const double* n, int Nx, int Ny, double h, double kappa, double B,
+                          double K) {
+  const double *n1 = n, *n2 = n + (size_t)Nx * Ny, *n3 = n + 2 * (size_t)Nx * Ny;
+  double E = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t a = (size_t)j * Nx + i;
+      for (int mu = 0; mu < 2; ++mu)
+        for (int k = 1; k <= 2; ++k) {
+          int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+          if (!inside(Nx, Ny, i2, j2)) continue;
+          if (!interior(Nx, Ny, i, j) && !interior(Nx, Ny, i2, j2)) continue;
+          size_t b = (size_t)j2 * Nx + i2;
+          double dx1 = n1[a] - n1[b], dx2 = n2[a] - n2[b], dx3 = n3[a] - n3[b];
+          double ex = 0.5 * Jw[k] * (dx1 * dx1 + dx2 * dx2 + dx3 * dx3);
+          /* e_mu . (n_a x n_b): x-component n2a n3b - n3a n2b; y-component n3a n1b - n1a n3b */
+          double cr = (mu == 0) ? (n2[a] * n3[b] - n3[a] * n2[b]) : (n3[a] * n1[b] - n1[a] * n3[b]);
+          E += ex - 2.0 * kappa * (h * h) * cw(k, h) * cr;
+        }
+      if (interior(Nx, Ny, i, j))
+        E += (h * h) * (B * (1.0 - n3[a]) + K * (1.0 - n3[a] * n3[a]));
+    }
+  return E;
+}
+
+/* Site form of the same energy (DESIGN R3): for i in I, neighbours j = i + k mu,
+ * k = +1,-1,+2,-2, weight w(j) = 1 if j interior, 2 if j in the halo,
+ *   e_i = sum_mu sum_k w(j) [ J_|k|/(4h^2) |n_i-n_j|^2 + kappa c_k n_i.(e_mu x n_j) ]
+ *         + B(1-n3) + K(1-n3^2),   c_{-k} = -c_k,
+ *   n_i.(e_x x n_j) = n_i3 n_j2 - n_i2 n_j3 ,  n_i.(e_y x n_j) = n_i1 n_j3 - n_i3 n_j1. */
+static double cm_site_energy(const double* n, int Nx, int Ny, int j, int i, double h, double kappa,
+                             double B, double K) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *n1 = n, *n2 = n + P, *n3 = n + 2 * P;
+  static const int ks[4] = {1, -1, 2, -2};
+  size_t a = (size_t)j * Nx + i;
+  double e = 0.0;
+  for (int mu = 0; mu < 2; ++mu)
+    for (int q = 0; q < 4; ++q) {
+      int k = ks[q], ak = k < 0 ? -k : k;
+      int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+      size_t b = (size_t)j2 * Nx + i2;
+      double w = interior(Nx, Ny, i2, j2) ? 1.0 : 2.0;
+      double ck = (k > 0 ? 1.0 : -1.0) * cw(ak, h);
+      double dx1 = n1[a] - n1[b], dx2 = n2[a] - n2[b], dx3 = n3[a] - n3[b];
+      double ex = Jw[ak] / (4.0 * (h * h)) * (dx1 * dx1 + dx2 * dx2 + dx3 * dx3);
+      double cr = (mu == 0) ? (n3[a] * n2[b] - n2[a] * n3[b]) : (n1[a] * n3[b] - n3[a] * n1[b]);
+      e += w * (ex + kappa * ck * cr);
+    }
+  e += B * (1.0 - n3[a]) + K * (1.0 - n3[a] * n3[a]);
+  return e;
+}
+
+
+/* Charge density (BASELINE config 2: Q = (1/4pi) sum n.(d1 n x d2 n) h^2; "conserved
+ * topological charge"): q = (1/4pi) n.(Dx n x Dy n) with eq. (1). */
+static double cm_site_charge(const double* n, int Nx, int Ny, int j, int i, double h) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *n1 = n, *n2 = n + P, *n3 = n + 2 * P;
+  size_t a = (size_t)j * Nx + i;
+  double x1 = Dx(n1, Nx, j, i, h), x2 = Dx(n2, Nx, j, i, h), x3 = Dx(n3, Nx, j, i, h);
+  double y1 = Dy(n1, Nx, j, i, h), y2 = Dy(n2, Nx, j, i, h), y3 = Dy(n3, Nx, j, i, h);
+  double c1 = x2 * y3 - x3 * y2, c2 = x3 * y1 - x1 * y3, c3 = x1 * y2 - x2 * y1;
+  return (1.0 / (4.0 * PI)) * ((n1[a] * c1 + n2[a] * c2) + n3[a] * c3);
+}
+
+/* Functional derivative G = (1/h^2) dE_h/dn_i at an interior site (DESIGN R2,R5): the
+ * Euler-Lagrange expression discretised with eq. (1) and (2),
+ *   G = -(Lx n + Ly n) + 2 kappa ( Dy n3, -Dx n3, Dx n2 - Dy n1 ) - (B + 2K n3) e3 . */
+static void cm_site_gradient(const double* n, int Nx, int Ny, int j, int i, double h, double kappa,
+                             double B, double K, double G[3]) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *n1 = n, *n2 = n + P, *n3 = n + 2 * P;
+  size_t a = (size_t)j * Nx + i;
+  G[0] = -(Lx(n1, Nx, j, i, h) + Ly(n1, Nx, j, i, h)) + 2.0 * kappa * Dy(n3, Nx, j, i, h);
+  G[1] = -(Lx(n2, Nx, j, i, h) + Ly(n2, Nx, j, i, h)) - 2.0 * kappa * Dx(n3, Nx, j, i, h);
+  G[2] = -(Lx(n3, Nx, j, i, h) + Ly(n3, Nx, j, i, h)) +
+         2.0 * kappa * (Dx(n2, Nx, j, i, h) - Dy(n1, Nx, j, i, h)) - (B + 2.0 * K * n3[a]);
+}
+
+/* ------------------------------------------------------------ abelian Higgs */
+/* Functional (Table 2 with u = 1; BASELINE config 3):
+ *   e = 1/2 |D phi|^2 + 1/2 (d1 A2 - d2 A1)^2 + (lambda/8)(1-|phi|^2)^2 ,  D = d - iA.
+ * Components: f[0]=Re phi, f[1]=Im phi, f[2]=A1, f[3]=A2.
+ * Expanded: 1/2|d phi|^2 - A_mu Im(phi* d_mu phi) + 1/2|A|^2|phi|^2 + 1/2(d1A2)^2
+ * + 1/2(d2A1)^2 - (d1A2)(d2A1) + potential.  Discrete energy (DESIGN R1,R3) = every
+ * elementary product that touches an interior site, counted once:
+ *  bonds (i, j=i+k mu), k in {1,2}, >=1 end interior:
+ *      J_k/2 |phi_i-phi_j|^2  -  h^2 c_k (A_mu,i + A_mu,j) Im(phi_i* phi_j)
+ *      + J_k/2 (A2_i-A2_j)^2 on x-bonds ;  + J_k/2 (A1_i-A1_j)^2 on y-bonds
+ *  pairs (a = s+k x, b = s+l y), k,l in {+-1,+-2}, a,b in the lattice, >=1 interior:
+ *      - h^2 c_k c_l A2_a A1_b
+ *  sites i in I:  h^2 [ 1/2 (A1^2+A2^2) rho + (lambda/8)(1-rho)^2 ],  rho = |phi|^2. */
+double orc_ah_energy_bond(const double* f, int Nx, int Ny, double h, double lambda) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *p1 = f, *p2 = f + P, *A1 = f + 2 * P, *A2 = f + 3 * P;
+  double E = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t a = (size_t)j * Nx + i;
+      for (int mu = 0; mu < 2; ++mu)
+        for (int k = 1; k <= 2; ++k) {
+          int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+          if (!inside(Nx, Ny, i2, j2)) continue;
+          if (!interior(Nx, Ny, i, j) && !interior(Nx, Ny, i2, j2)) continue;
+          size_t b = (size_t)j2 * Nx + i2;
+          double d1r = p1[a] - p1[b], d2r = p2[a] - p2[b];
+          const double* Am = (mu == 0) ? A1 : A2;  /* A_mu along the bond            */
+          const double* At = (mu == 0) ? A2 : A1;  /* transverse component           */
+          double dA = At[a] - At[b];
+          double im = p1[a] * p2[b] - p2[a] * p1[b]; /* Im(phi_a* phi_b) */
+          E += 0.5 * Jw[k] * (d1r * d1r + d2r * d2r) - (h * h) * cw(k, h) * (Am[a] + Am[b]) * im +
+               0.5 * Jw[k] * (dA * dA);
+        }
+      if (interior(Nx, Ny, i, j)) {
+        double rho = p1[a] * p1[a] + p2[a] * p2[a];
+        E += (h * h) * (0.5 * (A1[a] * A1[a] + A2[a] * A2[a]) * rho +
+                        (lambda / 8.0) * (1.0 - rho) * (1.0 - rho));
+      }
+      /* mixed term: (i,j) plays the role of s; a' = s + k x, b' = s + l y */
+      for (int k = -2; k <= 2; ++k)
+        for (int l = -2; l <= 2; ++l) {
+          if (k == 0 || l == 0) continue;
+          int ia = i + k, jb = j + l;
+          if (!inside(Nx, Ny, ia, j) || !inside(Nx, Ny, i, jb)) continue;
+          if (!interior(Nx, Ny, ia, j) && !interior(Nx, Ny, i, jb)) continue;
+          double ck = (k > 0 ? 1.0 : -1.0) * cw(k < 0 ? -k : k, h);
+          double cl = (l > 0 ? 1.0 : -1.0) * cw(l < 0 ? -l : l, h);
+          E -= (h * h) * ck * cl * A2[(size_t)j * Nx + ia] * A1[(size_t)jb * Nx + i];
+        }
+    }
+  return E;
+}
+
+/* Site form (DESIGN R3); w(.) = 1 interior, 2 halo:
+ *  e_i = 1/2(A1^2+A2^2) rho + (lambda/8)(1-rho)^2
+ *      + sum_mu sum_{k=+1,-1,+2,-2} w(j) [ J_|k|/(4h^2) |phi_i-phi_j|^2
+ *              - 1/2 c_k (A_mu,i + A_mu,j) Im(phi_i* phi_j) + J_|k|/(4h^2) (At_i - At_j)^2 ]
+ *      - 1/2 sum_{k,l} c_k c_l [ A2_i w(i+(-k,+l)) A1(i+(-k,+l)) + A1_i w(i+(+k,-l)) A2(i+(+k,-l)) ] */
+static double ah_site_energy(const double* f, int Nx, int Ny, int j, int i, double h,
+                             double lambda) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *p1 = f, *p2 = f + P, *A1 = f + 2 * P, *A2 = f + 3 * P;
+  static const int ks[4] = {1, -1, 2, -2};
+  size_t a = (size_t)j * Nx + i;
+  double rho = p1[a] * p1[a] + p2[a] * p2[a];
+  double e = 0.5 * (A1[a] * A1[a] + A2[a] * A2[a]) * rho + (lambda / 8.0) * (1.0 - rho) * (1.0 - rho);
+  for (int mu = 0; mu < 2; ++mu)
+    for (int q = 0; q < 4; ++q) {
+      int k = ks[q], ak = k < 0 ? -k : k;
+      int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+      size_t b = (size_t)j2 * Nx + i2;
+      double w = interior(Nx, Ny, i2, j2) ? 1.0 : 2.0;
+      double ck = (k > 0 ? 1.0 : -1.0) * cw(ak, h);
+      const double* Am = (mu == 0) ? A1 : A2;
+      const double* At = (mu == 0) ? A2 : A1;
+      double d1r = p1[a] - p1[b], d2r = p2[a] - p2[b], dA = At[a] - At[b];
+      double im = p1[a] * p2[b] - p2[a] * p1[b];
+      e += w * (Jw[ak] / (4.0 * (h * h)) * (d1r * d1r + d2r * d2r) -
+                0.5 * ck * (Am[a] + Am[b]) * im + Jw[ak] / (4.0 * (h * h)) * (dA * dA));
+    }
+  double mix = 0.0;
+  for (int qk = 0; qk < 4; ++qk)
+    for (int ql = 0; ql < 4; ++ql) {
+      int k = ks[qk], l = ks[ql];
+      double ck = (k > 0 ? 1.0 : -1.0) * cw(k < 0 ? -k : k, h);
+      double cl = (l > 0 ? 1.0 : -1.0) * cw(l < 0 ? -l : l, h);
+      int ib = i - k, jb = j + l; /* partner A1 site of A2_i */
+      int ic = i + k, jc = j - l; /* partner A2 site of A1_i */
+      double wb = interior(Nx, Ny, ib, jb) ? 1.0 : 2.0;
+      double wc = interior(Nx, Ny, ic, jc) ? 1.0 : 2.0;
+      mix += ck * cl * (A2[a] * (wb * A1[(size_t)jb * Nx + ib]) + A1[a] * (wc * A2[(size_t)jc * Nx + ic]));
+    }
+  return e - 0.5 * mix;
+}
+
+/* Diagnostic "literal" energy density with eq. (1) only (DESIGN R1, used for the
+ * Bogomolny / closed-form pins, never for the arrest):
+ *  1/2 sum_mu [(D_mu p1 + A_mu p2)^2 + (D_mu p2 - A_mu p1)^2] + 1/2 (Dx A2 - Dy A1)^2 + pot. */
+static double ah_site_energy_literal(const double* f, int Nx, int Ny, int j, int i, double h,
+                                     double lambda) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *p1 = f, *p2 = f + P, *A1 = f + 2 * P, *A2 = f + 3 * P;
+  size_t a = (size_t)j * Nx + i;
+  double rho = p1[a] * p1[a] + p2[a] * p2[a];
+  double r1x = Dx(p1, Nx, j, i, h) + A1[a] * p2[a], r2x = Dx(p2, Nx, j, i, h) - A1[a] * p1[a];
+  double r1y = Dy(p1, Nx, j, i, h) + A2[a] * p2[a], r2y = Dy(p2, Nx, j, i, h) - A2[a] * p1[a];
+  double Bz = Dx(A2, Nx, j, i, h) - Dy(A1, Nx, j, i, h);
+  return 0.5 * (r1x * r1x + r2x * r2x + r1y * r1y + r2y * r2y) + 0.5 * Bz * Bz +
+         (lambda / 8.0) * (1.0 - rho) * (1.0 - rho);
+}
+
+/* Vortex-number density (DESIGN R9): flux / 2pi with eq. (1). */
+static double ah_site_charge(const double* f, int Nx, int Ny, int j, int i, double h) {
+  const size_t P = (size_t)Nx * Ny;
+  return (1.0 / (2.0 * PI)) * (Dx(f + 3 * P, Nx, j, i, h) - Dy(f + 2 * P, Nx, j, i, h));
+}
+
+/* G = (1/h^2) dE_h/d(field) at an interior site (DESIGN R2); D_mu(A_mu phi) is the
+ * stencil applied to the product evaluated at the neighbour sites:
+ *  G_p1 = -L p1 - sum_mu [ D_mu(A_mu p2) + A_mu D_mu p2 ] + |A|^2 p1 - (lambda/2)(1-rho) p1
+ *  G_p2 = -L p2 + sum_mu [ D_mu(A_mu p1) + A_mu D_mu p1 ] + |A|^2 p2 - (lambda/2)(1-rho) p2
+ *  G_A1 = -Ly A1 + DxDy A2 + p2 Dx p1 - p1 Dx p2 + A1 rho
+ *  G_A2 = -Lx A2 + DxDy A1 + p2 Dy p1 - p1 Dy p2 + A2 rho */
+static double Dx_prod(const double* u, const double* v, int Nx, int j, int i, double h) {
+  const double *p = u + (size_t)j * Nx + i, *q = v + (size_t)j * Nx + i;
+  return d1(p[-2] * q[-2], p[-1] * q[-1], p[1] * q[1], p[2] * q[2], h);
+}
+static double Dy_prod(const double* u, const double* v, int Nx, int j, int i, double h) {
+  const double *p = u + (size_t)j * Nx + i, *q = v + (size_t)j * Nx + i;
+  return d1(p[-2 * Nx] * q[-2 * Nx], p[-Nx] * q[-Nx], p[Nx] * q[Nx], p[2 * Nx] * q[2 * Nx], h);
+}
+static void ah_site_gradient(const double* f, int Nx, int Ny, int j, int i, double h, double lambda,
+                             double G[4]) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *p1 = f, *p2 = f + P, *A1 = f + 2 * P, *A2 = f + 3 * P;
+  size_t a = (size_t)j * Nx + i;
+  double rho = p1[a] * p1[a] + p2[a] * p2[a];
+  double AA = A1[a] * A1[a] + A2[a] * A2[a];
+  G[0] = -(Lx(p1, Nx, j, i, h) + Ly(p1, Nx, j, i, h)) -
+         ((Dx_prod(A1, p2, Nx, j, i, h) + A1[a] * Dx(p2, Nx, j, i, h)) +
+          (Dy_prod(A2, p2, Nx, j, i, h) + A2[a] * Dy(p2, Nx, j, i, h))) +
+         AA * p1[a] - (lambda / 2.0) * (1.0 - rho) * p1[a];
+  G[1] = -(Lx(p2, Nx, j, i, h) + Ly(p2, Nx, j, i, h)) +
+         ((Dx_prod(A1, p1, Nx, j, i, h) + A1[a] * Dx(p1, Nx, j, i, h)) +
+          (Dy_prod(A2, p1, Nx, j, i, h) + A2[a] * Dy(p1, Nx, j, i, h))) +
+         AA * p2[a] - (lambda / 2.0) * (1.0 - rho) * p2[a];
+  G[2] = -Ly(A1, Nx, j, i, h) + Dxy(A2, Nx, j, i, h) + p2[a] * Dx(p1, Nx, j, i, h) -
+         p1[a] * Dx(p2, Nx, j, i, h) + A1[a] * rho;
+  G[3] = -Lx(A2, Nx, j, i, h) + Dxy(A1, Nx, j, i, h) + p2[a] * Dy(p1, Nx, j, i, h) -
+         p1[a] * Dy(p2, Nx, j, i, h) + A2[a] * rho;
+}
+
+/* --------------------------------------------- whole-lattice evaluations (exported) */
+
+typedef struct {
+  int theory, Nx, Ny;
+  double h, kappa, B, K, lambda;
+} orc_model;
+
+static int ncomp(int theory) { return theory == ORC_CM ? 3 : 4; }
+
+/* Energy and charge with the canonical tree (DESIGN R10): E = (h*h) * tree(e_i),
+ * halo sites contribute +0.0.  dens_e / dens_q (Ny*Nx each) may be NULL.
+ * which_energy: 0 site form (the flow's E_h), 1 literal eq.(1) form (AH only). */
+void orc_energy_charge(const orc_model* m, const double* f, int which_energy, double* E, double* Q,
+                       double* dens_e, double* dens_q) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  size_t P = (size_t)Nx * Ny;
+  double* e = dens_e ? dens_e : (double*)malloc(P * sizeof(double));
+  double* q = dens_q ? dens_q : (double*)malloc(P * sizeof(double));
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t a = (size_t)j * Nx + i;
+      e[a] = 0.0;
+      q[a] = 0.0;
+      if (!interior(Nx, Ny, i, j)) continue;
+      if (m->theory == ORC_CM) {
+        e[a] = cm_site_energy(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K);
+        q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h);
+      } else {
+        e[a] = which_energy ? ah_site_energy_literal(f, Nx, Ny, j, i, m->h, m->lambda)
+                            : ah_site_energy(f, Nx, Ny, j, i, m->h, m->lambda);
+        q[a] = ah_site_charge(f, Nx, Ny, j, i, m->h);
+      }
+    }
+  *E = (m->h * m->h) * orc_tree_sum2d(e, Nx, Ny);
+  *Q = (m->h * m->h) * orc_tree_sum2d(q, Nx, Ny);
+  if (!dens_e) free(e);
+  if (!dens_q) free(q);
+}
+
+/* Raw gradient G on the interior (halo entries 0), [C][Ny][Nx]. */
+void orc_gradient(const orc_model* m, const double* f, double* G) {
+  const int Nx = m->Nx, Ny = m->Ny, C = ncomp(m->theory);
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      double g[4] = {0, 0, 0, 0};
+      if (interior(Nx, Ny, i, j)) {
+        if (m->theory == ORC_CM)
+          cm_site_gradient(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, g);
+        else
+          ah_site_gradient(f, Nx, Ny, j, i, m->h, m->lambda, g);
+      }
+      for (int c = 0; c < C; ++c) G[at(Nx, Ny, c, j, i)] = g[c];
+    }
+}
+
+/* Acceleration a = -Pi_f(G(f)) on the interior (eq. (3) with the tangent
+ * projection of PAPER.md:129+154, DESIGN R7): CM  a = -(G - (G.n) n), G.n = (G1n1+G2n2)+G3n3;
+ * AH  a = -G.  Halo entries 0. */
+void orc_accel(const orc_model* m, const double* f, double* a) {
+  const int Nx = m->Nx, Ny = m->Ny, C = ncomp(m->theory);
+  orc_gradient(m, f, a);
+#pragma omp parallel for schedule(static)
+  for (int j = 2; j < Ny - 2; ++j)
+    for (int i = 2; i < Nx - 2; ++i) {
+      if (m->theory == ORC_CM) {
+        double g1 = a[at(Nx, Ny, 0, j, i)], g2 = a[at(Nx, Ny, 1, j, i)], g3 = a[at(Nx, Ny, 2, j, i)];
+        double n1 = f[at(Nx, Ny, 0, j, i)], n2 = f[at(Nx, Ny, 1, j, i)], n3 = f[at(Nx, Ny, 2, j, i)];
+        double gn = (g1 * n1 + g2 * n2) + g3 * n3;
+        a[at(Nx, Ny, 0, j, i)] = -(g1 - gn * n1);
+        a[at(Nx, Ny, 1, j, i)] = -(g2 - gn * n2);
+        a[at(Nx, Ny, 2, j, i)] = -(g3 - gn * n3);
+      } else {
+        for (int c = 0; c < C; ++c) a[at(Nx, Ny, c, j, i)] = -a[at(Nx, Ny, c, j, i)];
+      }
+    }
+}
+
+/* ------------------------------------------------------------------ the flow */
+/* Arrested Newton flow: phi'' = -grad E (eq. 3), from rest,
+ * integrated as a first-order system with classical RK4, velocity set
+ * to zero whenever E[phi^{n+1}] > E[phi^n] (eq. 4), continuing from phi^{n+1}
+ * (PAPER.md:127); unit-length projection "during each Runge-Kutta stage"
+ * (PAPER.md:129+154).  RK4 for (phi, v) with the stage velocities eliminated (DESIGN R6):
+ *   k1 = a(phi)                       stage fields
+ *   k2 = a(phi + dt/2 v)                       phi2 = R(phi + dt/2 v)
+ *   k3 = a(phi + dt/2 v + dt^2/4 k1)           phi3 = R((phi + dt/2 v) + dt^2/4 a1)
+ *   k4 = a(phi + dt v + dt^2/2 k2)             phi4 = R((phi + dt v) + dt^2/2 a2)
+ *   phi' = phi + dt v + dt^2/6 (k1+k2+k3) ;  v' = v + dt/6 (k1 + 2k2 + 2k3 + k4). */
+
+typedef struct {
+  orc_model m;
+  double dt;
+  int C;
+  size_t P;
+  double *phi, *vel, *a1, *a2, *a3, *a4, *s;
+  double E, Q, KE, E_prev;
+  int v_is_zero, nonfinite;
+  int64_t n;
+  int64_t* log;
+  int64_t nlog, caplog;
+} orc_flow;
+
+orc_flow* orc_flow_create(const orc_model* m, double dt) {
+  orc_flow* s = (orc_flow*)calloc(1, sizeof(orc_flow));
+  s->m = *m;
+  s->dt = dt > 0.0 ? dt : 0.5 * m->h; /* C = dt/dx = 0.5 by default */
+  s->C = ncomp(m->theory);
+  s->P = (size_t)m->Nx * m->Ny;
+  size_t bytes = s->C * s->P * sizeof(double);
+  s->phi = (double*)calloc(1, bytes);
+  s->vel = (double*)calloc(1, bytes);
+  s->a1 = (double*)calloc(1, bytes);
+  s->a2 = (double*)calloc(1, bytes);
+  s->a3 = (double*)calloc(1, bytes);
+  s->a4 = (double*)calloc(1, bytes);
+  s->s = (double*)calloc(1, bytes);
+  s->caplog = 1024;
+  s->log = (int64_t*)malloc(s->caplog * sizeof(int64_t));
+  return s;
+}
+void orc_flow_destroy(orc_flow* s) {
+  free(s->phi); free(s->vel); free(s->a1); free(s->a2); free(s->a3); free(s->a4); free(s->s);
+  free(s->log);
+  free(s);
+}
+
+/* Evaluate a1, E, Q on the current field and take the arrest decision (eq. 4, strict >). */
+static void flow_evaluate(orc_flow* s) {
+  orc_accel(&s->m, s->phi, s->a1);
+  orc_energy_charge(&s->m, s->phi, 0, &s->E, &s->Q, NULL, NULL);
+  if (!isfinite(s->E)) s->nonfinite = 1;
+  s->v_is_zero = (s->E > s->E_prev);
+  if (s->v_is_zero) {
+    if (s->nlog == s->caplog) {
+      s->caplog *= 2;
+      s->log = (int64_t*)realloc(s->log, s->caplog * sizeof(int64_t));
+    }
+    s->log[s->nlog++] = s->n;
+  }
+  s->E_prev = s->E;
+}
+
+/* vel == NULL -> rest.  Halo velocities are ignored (treated as 0). */
+void orc_flow_set(orc_flow* s, const double* phi, const double* vel) {
+  const int Nx = s->m.Nx, Ny = s->m.Ny;
+  memcpy(s->phi, phi, s->C * s->P * sizeof(double));
+  memset(s->vel, 0, s->C * s->P * sizeof(double));
+  if (vel)
+    for (int c = 0; c < s->C; ++c)
+      for (int j = 2; j < Ny - 2; ++j)
+        for (int i = 2; i < Nx - 2; ++i) s->vel[at(Nx, Ny, c, j, i)] = vel[at(Nx, Ny, c, j, i)];
+  s->n = 0;
+  s->nlog = 0;
+  s->nonfinite = 0;
+  s->KE = 0.0;
+  s->E_prev = INFINITY;
+  flow_evaluate(s);
+}
+
+/* Stage field out = R(phi + alpha*vhat [+ beta*acc]) on the interior, frozen halo copied.
+ * R(m) = m/|m| for CM (|m| = sqrt((m1^2+m2^2)+m3^2), three divisions), identity for AH. */
+static void stage_field(const orc_flow* s, double alpha, double beta, const double* acc,
+                        double* out) {
+  const int Nx = s->m.Nx, Ny = s->m.Ny, C = s->C;
+  memcpy(out, s->phi, C * s->P * sizeof(double));
+#pragma omp parallel for schedule(static)
+  for (int j = 2; j < Ny - 2; ++j)
+    for (int i = 2; i < Nx - 2; ++i) {
+      double mm[4];
+      for (int c = 0; c < C; ++c) {
+        size_t a = at(Nx, Ny, c, j, i);
+        double vh = s->v_is_zero ? 0.0 : s->vel[a];
+        mm[c] = s->phi[a] + alpha * vh;
+        if (acc) mm[c] = mm[c] + beta * acc[a];
+      }
+      if (s->m.theory == ORC_CM) {
+        double nn = sqrt((mm[0] * mm[0] + mm[1] * mm[1]) + mm[2] * mm[2]);
+        for (int c = 0; c < 3; ++c) mm[c] = mm[c] / nn;
+      }
+      for (int c = 0; c < C; ++c) out[at(Nx, Ny, c, j, i)] = mm[c];
+    }
+}
+
+void orc_flow_step(orc_flow* s, int64_t k) {
+  const int Nx = s->m.Nx, Ny = s->m.Ny, C = s->C;
+  const double dt = s->dt, h = s->m.h;
+  const double hdt = 0.5 * dt, qdt2 = 0.25 * (dt * dt), hdt2 = 0.5 * (dt * dt),
+               sdt2 = (dt * dt) / 6.0, sdt = dt / 6.0;
+  double* ke = (double*)malloc(s->P * sizeof(double));
+  for (int64_t it = 0; it < k; ++it) {
+    stage_field(s, hdt, 0.0, NULL, s->s);   orc_accel(&s->m, s->s, s->a2);
+    stage_field(s, hdt, qdt2, s->a1, s->s); orc_accel(&s->m, s->s, s->a3);
+    stage_field(s, dt, hdt2, s->a2, s->s);  orc_accel(&s->m, s->s, s->a4);
+    memset(ke, 0, s->P * sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (int j = 2; j < Ny - 2; ++j)
+      for (int i = 2; i < Nx - 2; ++i) {
+        double f[4], u[4];
+        for (int c = 0; c < C; ++c) {
+          size_t a = at(Nx, Ny, c, j, i);
+          double vh = s->v_is_zero ? 0.0 : s->vel[a];
+          f[c] = (s->phi[a] + dt * vh) + sdt2 * ((s->a1[a] + s->a2[a]) + s->a3[a]);
+          u[c] = vh + sdt * ((s->a1[a] + 2.0 * s->a2[a]) + (2.0 * s->a3[a] + s->a4[a]));
+        }
+        if (s->m.theory == ORC_CM) {
+          double nn = sqrt((f[0] * f[0] + f[1] * f[1]) + f[2] * f[2]);
+          for (int c = 0; c < 3; ++c) f[c] = f[c] / nn;
+          double un = (u[0] * f[0] + u[1] * f[1]) + u[2] * f[2];
+          for (int c = 0; c < 3; ++c) u[c] = u[c] - un * f[c];
+        }
+        double v2 = 0.0;
+        for (int c = 0; c < C; ++c) {
+          s->phi[at(Nx, Ny, c, j, i)] = f[c];
+          s->vel[at(Nx, Ny, c, j, i)] = u[c];
+          v2 += u[c] * u[c];
+        }
+        ke[(size_t)j * Nx + i] = 0.5 * v2;
+      }
+    s->KE = (h * h) * orc_tree_sum2d(ke, Nx, Ny);
+    s->n += 1;
+    flow_evaluate(s);
+  }
+  free(ke);
+}
+
+void orc_flow_get(const orc_flow* s, double* phi, double* vel) {
+  if (phi) memcpy(phi, s->phi, s->C * s->P * sizeof(double));
+  if (vel) {
+    memcpy(vel, s->vel, s->C * s->P * sizeof(double));
+    if (s->v_is_zero) memset(vel, 0, s->C * s->P * sizeof(double)); /* arrested: v = 0 */
+  }
+}
+void orc_flow_scalars(const orc_flow* s, double* E, double* Q, double* KE, int64_t* n,
+                      int64_t* narrest, int* nonfinite, int* v_is_zero) {
+  *E = s->E; *Q = s->Q; *KE = s->KE; *n = s->n; *narrest = s->nlog;
+  *nonfinite = s->nonfinite; *v_is_zero = s->v_is_zero;
+}
+int64_t orc_flow_arrests(const orc_flow* s, int64_t* out, int64_t cap) {
+  int64_t c = s->nlog < cap ? s->nlog : cap;
+  memcpy(out, s->log, c * sizeof(int64_t));
+  return s->nlog;
+}
