@@ -1,0 +1,126 @@
+/*
+ * ss.h — C ABI of libss.so: the arrested-Newton-flow energy-minimisation step of
+ * arxiv/paper_2603_24370 (soliton_solver) on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers; "DESIGN Rn"
+ * = reading n in DESIGN.md where the paper is silent):
+ *   - a rectangular 2-D lattice with a frozen halo of width two and the 4th-order central
+ *     stencils of PAPER.md:100-109 (eq. 1, eq. 2);
+ *   - the discretised energy E_h, its exact gradient and the topological charge of
+ *       SS_THEORY_CHIRAL_MAGNET  n in S^2:  1/2|grad n|^2 + kappa n.(curl n) + B(1-n3) + K(1-n3^2)
+ *                                (PAPER.md:196 eq. 5, :327; DESIGN R1-R3),
+ *       SS_THEORY_ABELIAN_HIGGS  phi in C, A in R^2: 1/2|D phi|^2 + 1/2 (curl A)^2
+ *                                + (lambda/8)(1-|phi|^2)^2   (DESIGN R1-R3, R9);
+ *   - the arrested Newton flow phi'' = -grad E_h (eq. 3) integrated with
+ *     classical RK4, the unit-length projection applied in every stage
+ *     (PAPER.md:129+154), the velocity set to zero whenever E_h rises (eq. 4);
+ *   - device-resident reductions of E, Q and the kinetic energy in a fixed tree order
+ *     (DESIGN R10) that drive the arrest with no host synchronisation.
+ *
+ * Conventions
+ *   Lattice   Nx x Ny sites INCLUDING the halo (DESIGN R4); site (i,j), i fastest.
+ *             Interior = 2 <= i < Nx-2, 2 <= j < Ny-2.  Halo sites are frozen: supplied by
+ *             ss_set_fields and never written by a step.
+ *   Layout    field arrays are dense [batch][C][Ny][Nx] of `real` (double for SS_F64, float
+ *             for SS_F32), x fastest.  C = 3 (n1,n2,n3) for the chiral magnet, C = 4
+ *             (Re phi, Im phi, A1, A2) for Abelian Higgs.  Velocities have the same shape;
+ *             their halo entries are ignored on input and written as 0 on output.
+ *   Memory    every pointer named *_dev is DEVICE memory owned by the caller; every pointer
+ *             named *_host is HOST memory owned by the caller.  The library allocates no
+ *             device memory: all of its state lives in the caller's `workspace`
+ *             (ss_workspace_bytes), which must outlive the handle.  The caller also owns the
+ *             CUDA stream; all work is enqueued on it.
+ *   Errors    every call returns an SS_* status; nothing throws or aborts across the ABI.
+ *   Threads   a handle is not thread-safe; distinct handles are independent.
+ *   No CPU fallback exists: without a CUDA device ss_create returns SS_ERR_CUDA.
+ */
+#ifndef SS_H_
+#define SS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ss_solver ss_solver; /* opaque */
+
+enum { SS_THEORY_CHIRAL_MAGNET = 0, SS_THEORY_ABELIAN_HIGGS = 1 };
+enum { SS_F64 = 0, SS_F32 = 1 };
+enum {
+  SS_OK = 0,
+  SS_ERR_ARG = -1,         /* NULL pointer, bad size/enum, misaligned row length           */
+  SS_ERR_UNSUPPORTED = -2, /* valid request this build does not implement                   */
+  SS_ERR_CUDA = -3,        /* CUDA runtime failure (text via ss_strerror)                   */
+  SS_ERR_WORKSPACE = -4,   /* workspace NULL / too small / misaligned                       */
+  SS_ERR_STATE = -5,       /* stepping or reading before ss_set_fields                      */
+  SS_ERR_NONFINITE = -6    /* an energy became NaN/Inf (values are still written)           */
+};
+
+/* Integrators.  SS_RK4 is the paper's; others are reserved. */
+enum { SS_RK4 = 0 };
+
+typedef struct {
+  int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
+                           /* reductions, E, Q, KE and the arrest test are always fp64      */
+  int batch;               /* >= 1 independent lattices sharing Nx, Ny, h, dt               */
+  double dt;               /* <= 0 -> 0.5*h (Courant number C = 0.5)          */
+  double kappa, B, K;      /* chiral magnet: DMI, Zeeman field, uniaxial anisotropy         */
+  const double* B_batch;   /* optional HOST array[batch]: per-lattice B (overrides B)       */
+  double lambda;           /* Abelian Higgs coupling (critical at 1)                        */
+  void* workspace;         /* DEVICE memory, >= ss_workspace_bytes, 256-byte aligned        */
+  size_t workspace_bytes;
+  void* stream;            /* cudaStream_t owned by the caller; NULL = default stream       */
+  int64_t arrest_log_capacity; /* entries per lattice; 0 -> 4096; later arrests are counted */
+                               /* but not logged                                            */
+  int integrator;          /* SS_RK4                                                        */
+  int flags;               /* bit 0: launch kernels one by one instead of replaying the     */
+                           /* per-step CUDA graph (debugging; same results)                 */
+} ss_params;
+
+/* Bytes of device workspace ss_create needs for this problem; 0 on invalid arguments. */
+size_t ss_workspace_bytes(int theory, int Nx, int Ny, const ss_params* p);
+
+/* Create a solver (lattice, spacing, components and time step are fixed
+ * before any device buffer is carved).  Requires Nx, Ny >= 5; Nx even for SS_F64 and a
+ * multiple of 4 for SS_F32 (16-byte rows).  *out is NULL on failure. */
+int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_params* p);
+int ss_destroy(ss_solver* s);
+
+/* Load fields (halo included, frozen from now on) and velocities (NULL = from rest,
+ * PAPER.md:123) by device-to-device copies on the stream; resets the step counter and the
+ * arrest log, sets E_prev = +inf (step 0 cannot arrest) and evaluates a(phi), E, Q so that
+ * ss_energy / ss_charge are valid at once.  |n| = 1 is NOT enforced on input. */
+int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev);
+
+/* Copy the current fields / velocities out (either may be NULL).  After an arrested step
+ * the velocity reads as exactly 0. */
+int ss_get_fields(ss_solver* s, void* fields_dev, void* vel_dev);
+
+/* Enqueue k flow steps (asynchronous; no host synchronisation, the arrest of eq. 4 is
+ * decided on the device).  One step = RK4 stages 2-4 + update + projection, then the
+ * stencil pass on the new field (a, E, Q) and the arrest decision. */
+int ss_step(ss_solver* s, int64_t k);
+
+/* Scalar read-outs: synchronise the stream, then fill HOST arrays of length batch.
+ * Return SS_ERR_NONFINITE (after filling) if any lattice has a non-finite energy. */
+int ss_energy(ss_solver* s, double* E_host);  /* E_h of the current field                  */
+int ss_charge(ss_solver* s, double* Q_host);  /* CM: degree; AH: flux / 2 pi               */
+int ss_kinetic(ss_solver* s, double* KE_host); /* 1/2 h^2 sum |v|^2 of the last step,      */
+                                               /* before its arrest; 0 after ss_set_fields */
+/* steps_done: scalar; n_arrests, nonfinite: HOST arrays[batch]; any may be NULL. */
+int ss_status(ss_solver* s, int64_t* steps_done, int64_t* n_arrests, int* nonfinite);
+/* Arrest log of one lattice: the 1-based indices n+1 of the steps whose result raised the
+ * energy.  Writes min(count, cap) entries to steps_host, the total to *count. */
+int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int64_t* count);
+
+/* Number of kernel launches (graph nodes included) enqueued by this handle so far. */
+int64_t ss_launch_count(const ss_solver* s);
+
+const char* ss_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SS_H_ */

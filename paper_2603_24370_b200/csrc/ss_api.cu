@@ -1,0 +1,454 @@
+// Host side of libss.so: the C ABI of include/ss.h.  Handle, workspace carving, the per-step
+// CUDA graph (built with explicit kernel nodes so it can be replayed on any caller stream,
+// including the legacy default stream), and the scalar read-outs.
+#include "../../include/ss.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "ss_kernels.cuh"
+
+using namespace ss;
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "";
+
+inline bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA failure in %s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+#define CK(call)                                  \
+  do {                                            \
+    if (!cuda_ok((call), #call)) return SS_ERR_CUDA; \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Layout {
+  size_t field_bytes;  // one [batch][C][Ny][Nx] array
+  size_t part_bytes;   // one [batch][Ny][nseg] fp64 array
+  size_t rows_bytes;   // [batch][3][Ny]
+  size_t state_bytes, log_bytes, bb_bytes;
+  size_t off_phi[2], off_vel[2], off_a[3], off_part[3], off_rows, off_state, off_log, off_bb;
+  size_t total;
+  int nseg;
+};
+
+bool valid_shape(int theory, int Nx, int Ny, const ss_params* p) {
+  if (!p) return false;
+  if (theory != SS_THEORY_CHIRAL_MAGNET && theory != SS_THEORY_ABELIAN_HIGGS) return false;
+  if (p->dtype != SS_F64 && p->dtype != SS_F32) return false;
+  if (Nx < 5 || Ny < 5 || p->batch < 1) return false;
+  if (p->dtype == SS_F64 ? (Nx % 2 != 0) : (Nx % 4 != 0)) return false;
+  if (Nx > 16384 || Ny > 32768) return false;  // reduction tree limits (32 lanes x 8, 1024 x 32)
+  if (p->arrest_log_capacity < 0) return false;
+  return true;
+}
+
+Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
+  Layout L;
+  const int C = theory == SS_THEORY_CHIRAL_MAGNET ? 3 : 4;
+  const size_t R = p->dtype == SS_F64 ? 8 : 4;
+  const size_t cap = p->arrest_log_capacity > 0 ? (size_t)p->arrest_log_capacity : 4096;
+  L.nseg = (Nx + SEG - 1) / SEG;
+  L.field_bytes = align_up((size_t)p->batch * C * Ny * Nx * R);
+  L.part_bytes = align_up((size_t)p->batch * Ny * L.nseg * sizeof(double));
+  L.rows_bytes = align_up((size_t)p->batch * 3 * Ny * sizeof(double));
+  L.state_bytes = align_up((size_t)p->batch * sizeof(LatticeState));
+  L.log_bytes = align_up((size_t)p->batch * cap * sizeof(long long));
+  L.bb_bytes = align_up((size_t)p->batch * sizeof(double));
+  size_t o = 0;
+  for (int i = 0; i < 2; ++i) { L.off_phi[i] = o; o += L.field_bytes; }
+  for (int i = 0; i < 2; ++i) { L.off_vel[i] = o; o += L.field_bytes; }
+  for (int i = 0; i < 3; ++i) { L.off_a[i] = o; o += L.field_bytes; }
+  for (int i = 0; i < 3; ++i) { L.off_part[i] = o; o += L.part_bytes; }
+  L.off_rows = o; o += L.rows_bytes;
+  L.off_state = o; o += L.state_bytes;
+  L.off_log = o; o += L.log_bytes;
+  L.off_bb = o; o += L.bb_bytes;
+  L.total = o;
+  return L;
+}
+
+struct KernelNode {
+  void* func;
+  dim3 grid, block;
+  size_t smem;
+  std::vector<unsigned char> args;  // the single by-value argument struct
+};
+
+template <int THEORY, typename real>
+void* stage_func(int stage) {
+  switch (stage) {
+    case 1: return (void*)stage_kernel<THEORY, real, 1>;
+    case 2: return (void*)stage_kernel<THEORY, real, 2>;
+    case 3: return (void*)stage_kernel<THEORY, real, 3>;
+    default: return (void*)stage_kernel<THEORY, real, 4>;
+  }
+}
+void* stage_func(int theory, int dtype, int stage) {
+  if (theory == SS_THEORY_CHIRAL_MAGNET)
+    return dtype == SS_F64 ? stage_func<kCM, double>(stage) : stage_func<kCM, float>(stage);
+  return dtype == SS_F64 ? stage_func<kAH, double>(stage) : stage_func<kAH, float>(stage);
+}
+
+}  // namespace
+
+struct ss_solver {
+  int theory, dtype, C, Nx, Ny, batch;
+  double h, dt, kappa, B, K, lambda;
+  size_t R;
+  cudaStream_t stream;
+  char* ws;
+  Layout L;
+  long long log_cap;
+  int flags;
+  bool fields_set;
+  int cur;  // which ping-pong buffer holds (phi, v)
+  int64_t steps_done, launches;
+  std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
+  std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
+  cudaGraphExec_t step_exec[2];
+  std::vector<LatticeState> host_state;
+
+  void* phi(int i) const { return ws + L.off_phi[i]; }
+  void* vel(int i) const { return ws + L.off_vel[i]; }
+  void* acc(int i) const { return ws + L.off_a[i]; }
+  double* part(int i) const { return (double*)(ws + L.off_part[i]); }
+  LatticeState* state() const { return (LatticeState*)(ws + L.off_state); }
+};
+
+namespace {
+
+template <typename real>
+KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
+  StageArgs<real> a;
+  memset(&a, 0, sizeof(a));
+  const double dt = s->dt, h = s->h;
+  a.phi = (const real*)s->phi(cur);
+  a.vel = (const real*)s->vel(cur);
+  a.aprev = stage == 3 ? (const real*)s->acc(0) : (const real*)s->acc(1);  // stage 4: a2
+  a.aout = (real*)s->acc(stage == 1 ? 0 : stage == 2 ? 1 : 2);
+  a.a1 = (const real*)s->acc(0);
+  a.a3 = (const real*)s->acc(2);
+  a.phi_out = (real*)s->phi(cur ^ 1);
+  a.vel_out = (real*)s->vel(cur ^ 1);
+  a.part_e = s->part(0);
+  a.part_q = s->part(1);
+  a.part_ke = s->part(2);
+  a.state = s->state();
+  a.Bb = (const double*)(s->ws + s->L.off_bb);
+  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg;
+  a.plane = (long long)s->Nx * s->Ny;
+  // stage fields (DESIGN "flow step"): phi2 = R(phi + dt/2 v), phi3 = R((phi + dt/2 v) + dt^2/4 a1),
+  // phi4 = R((phi + dt v) + dt^2/2 a2)
+  a.alpha = real(stage == 4 ? dt : 0.5 * dt);
+  a.beta = real(stage == 3 ? 0.25 * (dt * dt) : 0.5 * (dt * dt));
+  a.dt = real(dt);
+  a.sdt2 = real((dt * dt) / 6.0);
+  a.sdt = real(dt / 6.0);
+  a.i12h = real(1.0 / (12.0 * h));
+  a.i12h2 = real(1.0 / (12.0 * h * h));
+  a.kappa = real(s->kappa);
+  a.K = real(s->K);
+  a.lambda = real(s->lambda);
+  KernelNode n;
+  n.func = stage_func(s->theory, s->dtype, stage);
+  n.grid = dim3((s->Nx + TX - 1) / TX, (s->Ny + TY - 1) / TY, s->batch);
+  n.block = dim3(BX, BY, 1);
+  n.smem = (size_t)s->C * TYP * TXP * sizeof(real);
+  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  return n;
+}
+
+KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
+  return s->dtype == SS_F64 ? make_stage_node<double>(s, stage, cur)
+                            : make_stage_node<float>(s, stage, cur);
+}
+
+void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>& out) {
+  ReduceArgs a;
+  memset(&a, 0, sizeof(a));
+  a.part_e = s->part(0);
+  a.part_q = s->part(1);
+  a.part_ke = s->part(2);
+  a.rows = (double*)(s->ws + s->L.off_rows);
+  a.state = s->state();
+  a.log = (long long*)(s->ws + s->L.off_log);
+  a.log_cap = s->log_cap;
+  a.Ny = s->Ny; a.nseg = s->L.nseg; a.advance = advance;
+  a.h2 = s->h * s->h;
+  KernelNode r;
+  r.func = (void*)row_reduce_kernel;
+  r.grid = dim3((s->Ny + 7) / 8, s->batch, 1);
+  r.block = dim3(256, 1, 1);
+  r.smem = 0;
+  r.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  out.push_back(r);
+  KernelNode f = r;
+  f.func = (void*)finalize_kernel;
+  f.grid = dim3(s->batch, 1, 1);
+  f.block = dim3(1024, 1, 1);
+  out.push_back(f);
+}
+
+int launch_nodes(ss_solver* s, std::vector<KernelNode>& nodes) {
+  for (auto& n : nodes) {
+    void* params[1] = {n.args.data()};
+    CK(cudaLaunchKernel(n.func, n.grid, n.block, params, n.smem, s->stream));
+    s->launches += 1;
+  }
+  return SS_OK;
+}
+
+int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* exec) {
+  cudaGraph_t g;
+  CK(cudaGraphCreate(&g, 0));
+  cudaGraphNode_t prev{};
+  bool have_prev = false;
+  for (auto& n : nodes) {
+    cudaKernelNodeParams kp;
+    memset(&kp, 0, sizeof(kp));
+    void* params[1] = {n.args.data()};
+    kp.func = n.func;
+    kp.gridDim = n.grid;
+    kp.blockDim = n.block;
+    kp.sharedMemBytes = (unsigned)n.smem;
+    kp.kernelParams = params;
+    cudaGraphNode_t node;
+    cudaError_t e = cudaGraphAddKernelNode(&node, g, have_prev ? &prev : nullptr, have_prev ? 1 : 0, &kp);
+    if (!cuda_ok(e, "cudaGraphAddKernelNode")) { cudaGraphDestroy(g); return SS_ERR_CUDA; }
+    prev = node;
+    have_prev = true;
+  }
+  cudaError_t e = cudaGraphInstantiate(exec, g, 0);
+  cudaGraphDestroy(g);
+  if (!cuda_ok(e, "cudaGraphInstantiate")) return SS_ERR_CUDA;
+  return SS_OK;
+}
+
+int read_state(ss_solver* s) {
+  CK(cudaMemcpyAsync(s->host_state.data(), s->state(), s->batch * sizeof(LatticeState),
+                     cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return SS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ss_workspace_bytes(int theory, int Nx, int Ny, const ss_params* p) {
+  if (!valid_shape(theory, Nx, Ny, p)) return 0;
+  return make_layout(theory, Nx, Ny, p).total;
+}
+
+int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_params* p) {
+  if (!out) return SS_ERR_ARG;
+  *out = nullptr;
+  if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
+  if (p->integrator != SS_RK4) return SS_ERR_UNSUPPORTED;
+  int ndev = 0;
+  if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
+    if (ndev == 0) snprintf(g_cuda_msg, sizeof(g_cuda_msg), "no CUDA device (libss has no CPU path)");
+    return SS_ERR_CUDA;
+  }
+  Layout L = make_layout(theory, Nx, Ny, p);
+  if (!p->workspace || p->workspace_bytes < L.total || ((uintptr_t)p->workspace & 255) != 0)
+    return SS_ERR_WORKSPACE;
+  ss_solver* s = new (std::nothrow) ss_solver();
+  if (!s) return SS_ERR_ARG;
+  s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_CHIRAL_MAGNET ? 3 : 4;
+  s->Nx = Nx; s->Ny = Ny; s->batch = p->batch; s->h = h;
+  s->dt = p->dt > 0.0 ? p->dt : 0.5 * h;
+  s->kappa = p->kappa; s->B = p->B; s->K = p->K; s->lambda = p->lambda;
+  s->R = p->dtype == SS_F64 ? 8 : 4;
+  s->stream = (cudaStream_t)p->stream;
+  s->ws = (char*)p->workspace;
+  s->L = L;
+  s->log_cap = p->arrest_log_capacity > 0 ? p->arrest_log_capacity : 4096;
+  s->flags = p->flags;
+  s->fields_set = false;
+  s->cur = 0;
+  s->steps_done = 0; s->launches = 0;
+  s->step_exec[0] = s->step_exec[1] = nullptr;
+  s->host_state.resize(s->batch);
+
+  std::vector<double> bb(s->batch, p->B);
+  if (p->B_batch) bb.assign(p->B_batch, p->B_batch + s->batch);
+  cudaError_t e = cudaMemcpyAsync(s->ws + L.off_bb, bb.data(), s->batch * sizeof(double),
+                                  cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);  // bb is a local
+  if (!cuda_ok(e, "upload B_batch")) { delete s; return SS_ERR_CUDA; }
+
+  for (int stage = 1; stage <= 4; ++stage) {
+    void* f = stage_func(theory, p->dtype, stage);
+    e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)((size_t)s->C * TYP * TXP * s->R));
+    if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+  }
+  for (int cur = 0; cur < 2; ++cur) {
+    auto& st = s->step_nodes[cur];
+    st.push_back(make_stage_node(s, 2, cur));
+    st.push_back(make_stage_node(s, 3, cur));
+    st.push_back(make_stage_node(s, 4, cur));
+    st.push_back(make_stage_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
+    make_reduce_nodes(s, 1, st);
+    auto& ev = s->eval_nodes[cur];
+    ev.push_back(make_stage_node(s, 1, cur));
+    make_reduce_nodes(s, 0, ev);
+    if (!(s->flags & 1)) {
+      int rc = build_graph(s, st, &s->step_exec[cur]);
+      if (rc != SS_OK) { ss_destroy(s); return rc; }
+    }
+  }
+  *out = s;
+  return SS_OK;
+}
+
+int ss_destroy(ss_solver* s) {
+  if (!s) return SS_ERR_ARG;
+  for (int i = 0; i < 2; ++i)
+    if (s->step_exec[i]) cudaGraphExecDestroy(s->step_exec[i]);
+  delete s;
+  return SS_OK;
+}
+
+int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev) {
+  if (!s || !fields_dev) return SS_ERR_ARG;
+  const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
+  const long long planes = (long long)s->batch * s->C;
+  CK(cudaMemcpyAsync(s->phi(0), fields_dev, nbytes, cudaMemcpyDeviceToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->phi(1), fields_dev, nbytes, cudaMemcpyDeviceToDevice, s->stream));
+  CK(cudaMemsetAsync(s->vel(0), 0, nbytes, s->stream));
+  CK(cudaMemsetAsync(s->vel(1), 0, nbytes, s->stream));
+  if (vel_dev) {
+    if (s->dtype == SS_F64)
+      copy_interior_kernel<double><<<1184, 256, 0, s->stream>>>((double*)s->vel(0), (const double*)vel_dev,
+                                                                 s->Nx, s->Ny, planes);
+    else
+      copy_interior_kernel<float><<<1184, 256, 0, s->stream>>>((float*)s->vel(0), (const float*)vel_dev,
+                                                                s->Nx, s->Ny, planes);
+    s->launches += 1;
+  }
+  for (int i = 0; i < 3; ++i) CK(cudaMemsetAsync(s->part(i), 0, s->L.part_bytes, s->stream));
+  init_state_kernel<<<(s->batch + 127) / 128, 128, 0, s->stream>>>(s->state(), s->batch);
+  s->launches += 1;
+  CK(cudaGetLastError());
+  s->cur = 0;
+  s->steps_done = 0;
+  s->fields_set = true;
+  return launch_nodes(s, s->eval_nodes[0]);
+}
+
+int ss_get_fields(ss_solver* s, void* fields_dev, void* vel_dev) {
+  if (!s) return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
+  if (fields_dev)
+    CK(cudaMemcpyAsync(fields_dev, s->phi(s->cur), nbytes, cudaMemcpyDeviceToDevice, s->stream));
+  if (vel_dev) {
+    const long long per = (long long)s->C * s->Ny * s->Nx;
+    if (s->dtype == SS_F64)
+      export_velocity_kernel<double><<<1184, 256, 0, s->stream>>>(
+          (double*)vel_dev, (const double*)s->vel(s->cur), s->state(), per, s->batch);
+    else
+      export_velocity_kernel<float><<<1184, 256, 0, s->stream>>>(
+          (float*)vel_dev, (const float*)s->vel(s->cur), s->state(), per, s->batch);
+    s->launches += 1;
+    CK(cudaGetLastError());
+  }
+  return SS_OK;
+}
+
+int ss_step(ss_solver* s, int64_t k) {
+  if (!s || k < 0) return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  for (int64_t it = 0; it < k; ++it) {
+    if (s->flags & 1) {
+      int rc = launch_nodes(s, s->step_nodes[s->cur]);
+      if (rc != SS_OK) return rc;
+    } else {
+      CK(cudaGraphLaunch(s->step_exec[s->cur], s->stream));
+      s->launches += (int64_t)s->step_nodes[s->cur].size();
+    }
+    s->cur ^= 1;
+    s->steps_done += 1;
+  }
+  return SS_OK;
+}
+
+static int read_scalar(ss_solver* s, double* out, int which) {
+  if (!s || !out) return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  int rc = read_state(s);
+  if (rc != SS_OK) return rc;
+  bool bad = false;
+  for (int b = 0; b < s->batch; ++b) {
+    const LatticeState& st = s->host_state[b];
+    out[b] = which == 0 ? st.E : which == 1 ? st.Q : st.KE;
+    bad |= st.nonfinite != 0;
+  }
+  return bad ? SS_ERR_NONFINITE : SS_OK;
+}
+int ss_energy(ss_solver* s, double* E_host) { return read_scalar(s, E_host, 0); }
+int ss_charge(ss_solver* s, double* Q_host) { return read_scalar(s, Q_host, 1); }
+int ss_kinetic(ss_solver* s, double* KE_host) { return read_scalar(s, KE_host, 2); }
+
+int ss_status(ss_solver* s, int64_t* steps_done, int64_t* n_arrests, int* nonfinite) {
+  if (!s) return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  int rc = read_state(s);
+  if (rc != SS_OK) return rc;
+  if (steps_done) *steps_done = s->steps_done;
+  bool bad = false;
+  for (int b = 0; b < s->batch; ++b) {
+    if (n_arrests) n_arrests[b] = s->host_state[b].n_arrests;
+    if (nonfinite) nonfinite[b] = s->host_state[b].nonfinite;
+    bad |= s->host_state[b].nonfinite != 0;
+  }
+  return bad ? SS_ERR_NONFINITE : SS_OK;
+}
+
+int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int64_t* count) {
+  if (!s || !count || lattice < 0 || lattice >= s->batch || cap < 0 || (cap > 0 && !steps_host))
+    return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  int rc = read_state(s);
+  if (rc != SS_OK) return rc;
+  const int64_t total = s->host_state[lattice].n_arrests;
+  *count = total;
+  int64_t n = total < s->log_cap ? total : s->log_cap;
+  if (n > cap) n = cap;
+  if (n > 0) {
+    static_assert(sizeof(long long) == sizeof(int64_t), "log entry size");
+    CK(cudaMemcpyAsync(steps_host, s->ws + s->L.off_log + (size_t)lattice * s->log_cap * 8, n * 8,
+                       cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  return SS_OK;
+}
+
+int64_t ss_launch_count(const ss_solver* s) { return s ? s->launches : 0; }
+
+const char* ss_strerror(int code) {
+  switch (code) {
+    case SS_OK: return "ok";
+    case SS_ERR_ARG: return "invalid argument";
+    case SS_ERR_UNSUPPORTED: return "unsupported request";
+    case SS_ERR_CUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA failure";
+    case SS_ERR_WORKSPACE: return "workspace missing, too small or misaligned";
+    case SS_ERR_STATE: return "fields not set";
+    case SS_ERR_NONFINITE: return "non-finite energy";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

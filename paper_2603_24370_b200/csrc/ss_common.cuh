@@ -1,0 +1,70 @@
+// Shared device-side definitions of libss.so (CUDA, sm_100a).  No code here is shared with
+// oracle/: the oracle is an independent plain-C statement of the same mathematics.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ss {
+
+constexpr int kCM = 0, kAH = 1;
+constexpr int HALO = 2;  // PAPER.md:102 "fourth-order ... stencils and halo width two"
+
+// Row segment of the canonical reduction tree (DESIGN R10): per-row partial sums are stored
+// for aligned segments of SEG consecutive x.  All stencil kernels use tiles SEG wide.
+constexpr int SEG = 64;
+
+// Per-lattice scalars kept on the device (PAPER.md:158 reductions; eq. 4 arrest state).
+struct LatticeState {
+  double E, Q, KE, E_prev;
+  long long n_arrests, step;
+  int v_is_zero, nonfinite;
+};
+
+template <typename real>
+struct StageArgs {
+  const real* phi;    // [batch][C][Ny][Nx] current field (halo frozen)
+  const real* vel;    // velocity
+  const real* aprev;  // acceleration entering the stage field (a1 for stage 3, a2 for stage 4)
+  real* aout;         // acceleration written by stages 1-3
+  const real* a1;     // stage 4 only
+  const real* a3;     // stage 4 only
+  real* phi_out;      // stage 4 only: phi^{n+1}
+  real* vel_out;      // stage 4 only: v^{n+1}
+  double* part_e;     // [batch][Ny][nseg] row-segment partial sums (stage 1)
+  double* part_q;
+  double* part_ke;    // (stage 4)
+  const LatticeState* state;
+  const double* Bb;   // [batch] Zeeman field per lattice
+  int Nx, Ny, nseg;
+  long long plane;    // Nx*Ny
+  real alpha, beta;   // stage field = R(phi + alpha*vhat + beta*aprev)
+  real dt, sdt2, sdt; // dt, dt^2/6, dt/6
+  real i12h, i12h2;   // 1/(12h), 1/(12h^2)
+  real kappa, K, lambda;
+};
+
+struct ReduceArgs {
+  const double* part_e;  // [batch][Ny][nseg]
+  const double* part_q;
+  const double* part_ke;
+  double* rows;          // [batch][3][Ny] row sums
+  LatticeState* state;
+  long long* log;        // [batch][log_cap]
+  long long log_cap;
+  int Ny, nseg, advance;
+  double h2;             // h*h
+};
+
+// Aligned pairwise tree over the 32 lanes of a warp (lane l holds element l):
+// xor-shuffles realise t[m] = t[2m] + t[2m+1] level by level because IEEE addition commutes.
+__device__ __forceinline__ double warp_tree(double v) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+template <typename real> __device__ __forceinline__ real rsqrt_(real x);
+template <> __device__ __forceinline__ double rsqrt_<double>(double x) { return rsqrt(x); }
+template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return rsqrtf(x); }
+
+}  // namespace ss

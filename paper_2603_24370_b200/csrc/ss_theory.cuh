@@ -1,0 +1,215 @@
+// Per-site mathematics of the two theories, written against a tile accessor
+// T(c, dy, dx) = component c of the (stage) field at offset (dx, dy) from the site.
+// Formulas: DESIGN.md "Discrete energies" (readings R1-R3, R9); stencils PAPER.md:104-109.
+#pragma once
+#include "ss_common.cuh"
+
+namespace ss {
+
+// weights of the halo rule in the site-form energy: 1 if the neighbour is interior, 2 if it
+// lies in the frozen halo (DESIGN R3).  Index: 0:+1, 1:-1, 2:+2, 3:-2.
+struct EdgeW {
+  int x[4], y[4];
+  __device__ __forceinline__ EdgeW(int gx, int gy, int Nx, int Ny) {
+    x[0] = (gx + 1 < Nx - HALO) ? 1 : 2;
+    x[1] = (gx - 1 >= HALO) ? 1 : 2;
+    x[2] = (gx + 2 < Nx - HALO) ? 1 : 2;
+    x[3] = (gx - 2 >= HALO) ? 1 : 2;
+    y[0] = (gy + 1 < Ny - HALO) ? 1 : 2;
+    y[1] = (gy - 1 >= HALO) ? 1 : 2;
+    y[2] = (gy + 2 < Ny - HALO) ? 1 : 2;
+    y[3] = (gy - 2 >= HALO) ? 1 : 2;
+  }
+};
+
+// eq. (1) numerators: 12h * D f = 8 (f+1 - f-1) - (f+2 - f-2)
+template <typename real>
+__device__ __forceinline__ real d1n(real fm2, real fm1, real fp1, real fp2) {
+  return real(8) * (fp1 - fm1) - (fp2 - fm2);
+}
+
+template <typename real, typename Tile>
+__device__ __forceinline__ real Dxn(const Tile& T, int c) {
+  return d1n<real>(T(c, 0, -2), T(c, 0, -1), T(c, 0, 1), T(c, 0, 2));
+}
+template <typename real, typename Tile>
+__device__ __forceinline__ real Dyn(const Tile& T, int c) {
+  return d1n<real>(T(c, -2, 0), T(c, -1, 0), T(c, 1, 0), T(c, 2, 0));
+}
+// eq. (2) numerators: 12h^2 * Lx f, 12h^2 * Ly f
+template <typename real, typename Tile>
+__device__ __forceinline__ real Lxn(const Tile& T, int c) {
+  return real(16) * (T(c, 0, 1) + T(c, 0, -1)) - (T(c, 0, 2) + T(c, 0, -2)) - real(30) * T(c, 0, 0);
+}
+template <typename real, typename Tile>
+__device__ __forceinline__ real Lyn(const Tile& T, int c) {
+  return real(16) * (T(c, 1, 0) + T(c, -1, 0)) - (T(c, 2, 0) + T(c, -2, 0)) - real(30) * T(c, 0, 0);
+}
+// (12h)^2 * DxDy f on the 4x4 box of corner neighbours; W(dy,dx) optional weights
+template <typename real, typename Tile>
+__device__ __forceinline__ real Dxyn(const Tile& T, int c) {
+  real col[4];
+  const int ks[4] = {-2, -1, 1, 2};
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    col[q] = d1n<real>(T(c, -2, ks[q]), T(c, -1, ks[q]), T(c, 1, ks[q]), T(c, 2, ks[q]));
+  return d1n<real>(col[0], col[1], col[2], col[3]);
+}
+
+// ------------------------------------------------------------------ chiral magnet
+template <typename real>
+struct CM {
+  static constexpr int C = 3;
+
+  // a = -(G - (G.n) n),  G = -(Lx+Ly) n + 2 kappa (Dy n3, -Dx n3, Dx n2 - Dy n1) - (B + 2K n3) e3
+  template <typename Tile>
+  __device__ __forceinline__ static void accel(const Tile& T, const StageArgs<real>& p, real B,
+                                               real a[3]) {
+    const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
+    const real k2 = real(2) * p.kappa * p.i12h;
+    real G1 = -(Lxn<real>(T, 0) + Lyn<real>(T, 0)) * p.i12h2 + k2 * Dyn<real>(T, 2);
+    real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 - k2 * Dxn<real>(T, 2);
+    real G3 = -(Lxn<real>(T, 2) + Lyn<real>(T, 2)) * p.i12h2 +
+              k2 * (Dxn<real>(T, 1) - Dyn<real>(T, 0)) - (B + real(2) * p.K * n3);
+    const real gn = (G1 * n1 + G2 * n2) + G3 * n3;
+    a[0] = gn * n1 - G1;
+    a[1] = gn * n2 - G2;
+    a[2] = gn * n3 - G3;
+  }
+
+  // site-form energy density and charge density at an interior site
+  template <typename Tile>
+  __device__ __forceinline__ static void densities(const Tile& T, const StageArgs<real>& p, real B,
+                                                   const EdgeW& w, real& e, real& q) {
+    const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
+    const int ks[4] = {1, -1, 2, -2};
+    const real J4[4] = {real(4) * p.i12h2, real(4) * p.i12h2, real(-0.25) * p.i12h2,
+                        real(-0.25) * p.i12h2};  // J_|k| / (4 h^2)
+    const real ck[4] = {real(8) * p.i12h, real(-8) * p.i12h, -p.i12h, p.i12h};
+    real acc = real(0);
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      {  // x neighbour
+        const real m1 = T(0, 0, ks[s]), m2 = T(1, 0, ks[s]), m3 = T(2, 0, ks[s]);
+        const real d1 = n1 - m1, d2 = n2 - m2, d3 = n3 - m3;
+        const real ex = J4[s] * (d1 * d1 + d2 * d2 + d3 * d3);
+        const real cr = n3 * m2 - n2 * m3;  // n_i . (e_x x n_j)
+        acc += real(w.x[s]) * (ex + p.kappa * ck[s] * cr);
+      }
+      {  // y neighbour
+        const real m1 = T(0, ks[s], 0), m2 = T(1, ks[s], 0), m3 = T(2, ks[s], 0);
+        const real d1 = n1 - m1, d2 = n2 - m2, d3 = n3 - m3;
+        const real ex = J4[s] * (d1 * d1 + d2 * d2 + d3 * d3);
+        const real cr = n1 * m3 - n3 * m1;  // n_i . (e_y x n_j)
+        acc += real(w.y[s]) * (ex + p.kappa * ck[s] * cr);
+      }
+    }
+    e = acc + B * (real(1) - n3) + p.K * (real(1) - n3 * n3);
+    // q = (1/4pi) n . (Dx n x Dy n)
+    const real x1 = Dxn<real>(T, 0), x2 = Dxn<real>(T, 1), x3 = Dxn<real>(T, 2);
+    const real y1 = Dyn<real>(T, 0), y2 = Dyn<real>(T, 1), y3 = Dyn<real>(T, 2);
+    const real c1 = x2 * y3 - x3 * y2, c2 = x3 * y1 - x1 * y3, c3 = x1 * y2 - x2 * y1;
+    q = real(0.07957747154594767) * (p.i12h * p.i12h) * ((n1 * c1 + n2 * c2) + n3 * c3);
+  }
+
+  // R(m) = m / |m|
+  __device__ __forceinline__ static void project_field(real m[3]) {
+    const real r = rsqrt_<real>((m[0] * m[0] + m[1] * m[1]) + m[2] * m[2]);
+    m[0] *= r; m[1] *= r; m[2] *= r;
+  }
+  // v <- u - (u.n) n
+  __device__ __forceinline__ static void project_velocity(real u[3], const real n[3]) {
+    const real un = (u[0] * n[0] + u[1] * n[1]) + u[2] * n[2];
+    u[0] -= un * n[0]; u[1] -= un * n[1]; u[2] -= un * n[2];
+  }
+};
+
+// ------------------------------------------------------------------ abelian Higgs
+template <typename real>
+struct AH {
+  static constexpr int C = 4;  // 0: Re phi, 1: Im phi, 2: A1, 3: A2
+
+  template <typename Tile>
+  __device__ __forceinline__ static void accel(const Tile& T, const StageArgs<real>& p, real,
+                                               real a[4]) {
+    const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
+    const real rho = p1 * p1 + p2 * p2, AA = A1 * A1 + A2 * A2;
+    // S_mu,c = 12h * sum_k c_k (A_mu(i+k) + A_mu(i)) phi_c(i+k)
+    real Sx1, Sx2, Sy1, Sy2;
+    {
+      const real am2 = T(2, 0, -2) + A1, am1 = T(2, 0, -1) + A1, ap1 = T(2, 0, 1) + A1,
+                 ap2 = T(2, 0, 2) + A1;
+      Sx1 = d1n<real>(am2 * T(0, 0, -2), am1 * T(0, 0, -1), ap1 * T(0, 0, 1), ap2 * T(0, 0, 2));
+      Sx2 = d1n<real>(am2 * T(1, 0, -2), am1 * T(1, 0, -1), ap1 * T(1, 0, 1), ap2 * T(1, 0, 2));
+    }
+    {
+      const real am2 = T(3, -2, 0) + A2, am1 = T(3, -1, 0) + A2, ap1 = T(3, 1, 0) + A2,
+                 ap2 = T(3, 2, 0) + A2;
+      Sy1 = d1n<real>(am2 * T(0, -2, 0), am1 * T(0, -1, 0), ap1 * T(0, 1, 0), ap2 * T(0, 2, 0));
+      Sy2 = d1n<real>(am2 * T(1, -2, 0), am1 * T(1, -1, 0), ap1 * T(1, 1, 0), ap2 * T(1, 2, 0));
+    }
+    const real pot = real(0.5) * p.lambda * (real(1) - rho);
+    const real G1 = -(Lxn<real>(T, 0) + Lyn<real>(T, 0)) * p.i12h2 - (Sx2 + Sy2) * p.i12h +
+                    (AA - pot) * p1;
+    const real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 + (Sx1 + Sy1) * p.i12h +
+                    (AA - pot) * p2;
+    const real ii = p.i12h * p.i12h;
+    const real G3 = -Lyn<real>(T, 2) * p.i12h2 + Dxyn<real>(T, 3) * ii +
+                    (p2 * Dxn<real>(T, 0) - p1 * Dxn<real>(T, 1)) * p.i12h + A1 * rho;
+    const real G4 = -Lxn<real>(T, 3) * p.i12h2 + Dxyn<real>(T, 2) * ii +
+                    (p2 * Dyn<real>(T, 0) - p1 * Dyn<real>(T, 1)) * p.i12h + A2 * rho;
+    a[0] = -G1; a[1] = -G2; a[2] = -G3; a[3] = -G4;
+  }
+
+  template <typename Tile>
+  __device__ __forceinline__ static void densities(const Tile& T, const StageArgs<real>& p, real,
+                                                   const EdgeW& w, real& e, real& q) {
+    const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
+    const real rho = p1 * p1 + p2 * p2;
+    const int ks[4] = {1, -1, 2, -2};
+    const real J4[4] = {real(4) * p.i12h2, real(4) * p.i12h2, real(-0.25) * p.i12h2,
+                        real(-0.25) * p.i12h2};
+    const real ck[4] = {real(8) * p.i12h, real(-8) * p.i12h, -p.i12h, p.i12h};
+    real acc = real(0.5) * (A1 * A1 + A2 * A2) * rho +
+               real(0.125) * p.lambda * (real(1) - rho) * (real(1) - rho);
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      {  // x bond: A_mu = A1, transverse A2
+        const real q1 = T(0, 0, ks[s]), q2 = T(1, 0, ks[s]);
+        const real d1 = p1 - q1, d2 = p2 - q2, dA = A2 - T(3, 0, ks[s]);
+        const real im = p1 * q2 - p2 * q1;
+        acc += real(w.x[s]) * (J4[s] * (d1 * d1 + d2 * d2) -
+                               real(0.5) * ck[s] * (A1 + T(2, 0, ks[s])) * im + J4[s] * (dA * dA));
+      }
+      {  // y bond: A_mu = A2, transverse A1
+        const real q1 = T(0, ks[s], 0), q2 = T(1, ks[s], 0);
+        const real d1 = p1 - q1, d2 = p2 - q2, dA = A1 - T(2, ks[s], 0);
+        const real im = p1 * q2 - p2 * q1;
+        acc += real(w.y[s]) * (J4[s] * (d1 * d1 + d2 * d2) -
+                               real(0.5) * ck[s] * (A2 + T(3, ks[s], 0)) * im + J4[s] * (dA * dA));
+      }
+    }
+    // mixed term: + 1/2 [ A2 Wxy(A1) + A1 Wxy(A2) ], Wxy = weighted DxDy over corner sites
+    real W1 = real(0), W2 = real(0);
+#pragma unroll
+    for (int sk = 0; sk < 4; ++sk)
+#pragma unroll
+      for (int sl = 0; sl < 4; ++sl) {
+        const real wt = (w.x[sk] == 1 && w.y[sl] == 1) ? real(1) : real(2);
+        const real cc = ck[sk] * ck[sl] * wt;
+        W1 += cc * T(2, ks[sl], ks[sk]);
+        W2 += cc * T(3, ks[sl], ks[sk]);
+      }
+    e = acc + real(0.5) * (A2 * W1 + A1 * W2);
+    q = real(0.15915494309189535) * p.i12h * (Dxn<real>(T, 3) - Dyn<real>(T, 2));
+  }
+
+  __device__ __forceinline__ static void project_field(real*) {}
+  __device__ __forceinline__ static void project_velocity(real*, const real*) {}
+};
+
+template <int THEORY, typename real> struct TheoryOf;
+template <typename real> struct TheoryOf<kCM, real> { using type = CM<real>; };
+template <typename real> struct TheoryOf<kAH, real> { using type = AH<real>; };
+
+}  // namespace ss

@@ -1,0 +1,197 @@
+"""Thin ctypes binding of libss.so (include/ss.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: importing this module without the built library raises, and
+creating a solver without a CUDA device raises SSError(SS_ERR_CUDA).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libss.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_2603_24370_b200.build` "
+        "(nvcc, sm_100a).  There is no CPU fallback.")
+_lib = C.CDLL(LIB_PATH)
+
+THEORY_CHIRAL_MAGNET, THEORY_ABELIAN_HIGGS = 0, 1
+F64, F32 = 0, 1
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE = \
+    0, -1, -2, -3, -4, -5, -6
+FLAG_NO_GRAPH = 1
+
+EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
+           "ss_step", "ss_energy", "ss_charge", "ss_kinetic", "ss_status", "ss_arrests",
+           "ss_launch_count", "ss_strerror"]
+
+
+class ss_params(C.Structure):
+    _fields_ = [("dtype", C.c_int), ("batch", C.c_int), ("dt", C.c_double),
+                ("kappa", C.c_double), ("B", C.c_double), ("K", C.c_double),
+                ("B_batch", C.POINTER(C.c_double)), ("lam", C.c_double),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("stream", C.c_void_p), ("arrest_log_capacity", C.c_int64),
+                ("integrator", C.c_int), ("flags", C.c_int)]
+
+
+_dp = C.POINTER(C.c_double)
+_lib.ss_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(ss_params)]
+_lib.ss_workspace_bytes.restype = C.c_size_t
+_lib.ss_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double,
+                           C.POINTER(ss_params)]
+_lib.ss_destroy.argtypes = [C.c_void_p]
+_lib.ss_set_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.ss_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.ss_step.argtypes = [C.c_void_p, C.c_int64]
+for _n in ("ss_energy", "ss_charge", "ss_kinetic"):
+    getattr(_lib, _n).argtypes = [C.c_void_p, _dp]
+_lib.ss_status.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64),
+                           C.POINTER(C.c_int)]
+_lib.ss_arrests.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.c_int64,
+                            C.POINTER(C.c_int64)]
+_lib.ss_launch_count.argtypes = [C.c_void_p]
+_lib.ss_launch_count.restype = C.c_int64
+_lib.ss_strerror.argtypes = [C.c_int]
+_lib.ss_strerror.restype = C.c_char_p
+
+
+class SSError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__(f"{where}: {_lib.ss_strerror(code).decode()} ({code})")
+
+
+def strerror(code: int) -> str:
+    return _lib.ss_strerror(int(code)).decode()
+
+
+def _check(rc, where, allow=()):
+    if rc != OK and rc not in allow:
+        raise SSError(rc, where)
+    return rc
+
+
+def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags):
+    p = ss_params()
+    p.dtype, p.batch, p.dt = int(dtype), int(batch), float(dt)
+    p.kappa, p.B, p.K, p.lam = float(kappa), float(B), float(K), float(lam)
+    keep = None
+    if B_batch is not None:
+        keep = (C.c_double * int(batch))(*[float(x) for x in B_batch])
+        p.B_batch = C.cast(keep, _dp)
+    p.arrest_log_capacity = int(log_cap)
+    p.integrator, p.flags = 0, int(flags)
+    return p, keep
+
+
+def workspace_bytes(theory, Nx, Ny, dtype=F64, batch=1, log_cap=0) -> int:
+    p, _ = _params(dtype, batch, 0.0, 0, 0, 0, 0, None, log_cap, 0)
+    return _lib.ss_workspace_bytes(int(theory), int(Nx), int(Ny), C.byref(p))
+
+
+class Solver:
+    """ss_create ... ss_destroy around torch-owned device memory and the current torch stream."""
+
+    def __init__(self, theory, Nx, Ny, h, *, dtype=F64, batch=1, dt=0.0, kappa=0.0, B=0.0, K=0.0,
+                 lam=0.0, B_batch=None, log_cap=0, flags=0, device="cuda:0", stream=None):
+        self.theory, self.Nx, self.Ny, self.batch = int(theory), int(Nx), int(Ny), int(batch)
+        self.C = 3 if theory == THEORY_CHIRAL_MAGNET else 4
+        self.dtype = dtype
+        self.log_cap = int(log_cap) if log_cap else 4096
+        self.torch_dtype = torch.float64 if dtype == F64 else torch.float32
+        self.device = torch.device(device)
+        self._h = C.c_void_p()
+        p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags)
+        nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
+        if nbytes == 0:
+            raise SSError(ERR_ARG, "ss_workspace_bytes")
+        if not torch.cuda.is_available():
+            raise SSError(ERR_CUDA, "ss_create (no CUDA device; libss has no CPU path)")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        p.workspace = self.workspace.data_ptr()
+        p.workspace_bytes = nbytes
+        p.stream = self.stream.cuda_stream
+        with torch.cuda.device(self.device):
+            _check(_lib.ss_create(C.byref(self._h), self.theory, self.Nx, self.Ny, float(h),
+                                  C.byref(p)), "ss_create")
+
+    @property
+    def shape(self):
+        return (self.batch, self.C, self.Ny, self.Nx)
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            _lib.ss_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def _dev(self, t, name):
+        if t is None:
+            return None
+        if not (t.is_cuda and t.dtype == self.torch_dtype and t.is_contiguous()
+                and tuple(t.shape) == self.shape):
+            raise ValueError(f"{name}: need a contiguous {self.torch_dtype} CUDA tensor of shape "
+                             f"{self.shape}")
+        return C.c_void_p(t.data_ptr())
+
+    def set_fields(self, fields, vel=None):
+        _check(_lib.ss_set_fields(self._h, self._dev(fields, "fields"), self._dev(vel, "vel")),
+               "ss_set_fields")
+
+    def get_fields(self, want_vel=True):
+        f = torch.empty(self.shape, dtype=self.torch_dtype, device=self.device)
+        v = torch.empty_like(f) if want_vel else None
+        with torch.cuda.stream(self.stream):
+            _check(_lib.ss_get_fields(self._h, C.c_void_p(f.data_ptr()),
+                                      C.c_void_p(v.data_ptr()) if want_vel else None),
+                   "ss_get_fields")
+        return (f, v) if want_vel else f
+
+    def step(self, k=1):
+        _check(_lib.ss_step(self._h, int(k)), "ss_step")
+
+    def _scalar(self, fn, name, strict):
+        out = (C.c_double * self.batch)()
+        _check(fn(self._h, out), name, allow=() if strict else (ERR_NONFINITE,))
+        return [out[i] for i in range(self.batch)]
+
+    def energy(self, strict=True):
+        return self._scalar(_lib.ss_energy, "ss_energy", strict)
+
+    def charge(self, strict=True):
+        return self._scalar(_lib.ss_charge, "ss_charge", strict)
+
+    def kinetic(self, strict=True):
+        return self._scalar(_lib.ss_kinetic, "ss_kinetic", strict)
+
+    def status(self):
+        steps = C.c_int64()
+        na = (C.c_int64 * self.batch)()
+        nf = (C.c_int * self.batch)()
+        rc = _check(_lib.ss_status(self._h, C.byref(steps), na, nf), "ss_status",
+                    allow=(ERR_NONFINITE,))
+        return dict(steps=steps.value, n_arrests=list(na), nonfinite=list(nf), rc=rc)
+
+    def arrests(self, lattice=0):
+        cap = self.log_cap
+        buf = (C.c_int64 * cap)()
+        cnt = C.c_int64()
+        _check(_lib.ss_arrests(self._h, int(lattice), buf, cap, C.byref(cnt)), "ss_arrests")
+        return [int(buf[i]) for i in range(min(cnt.value, cap))], cnt.value
+
+    def launch_count(self) -> int:
+        return _lib.ss_launch_count(self._h)
+
+
+def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0) -> Solver:
+    """Solver configured from a workloads.Workload (sizes and parameters only)."""
+    return Solver(w.theory, w.Nx, w.Ny, w.h, dtype=dtype, batch=w.batch, dt=w.dt, kappa=w.kappa,
+                  B=w.B, K=w.K, lam=w.lam, B_batch=w.B_batch, log_cap=log_cap, flags=flags,
+                  device=device)

@@ -1,0 +1,206 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json's: fp64 fields max-abs <= 1e-11 over the first 100 steps with
+identical arrest-step indices; final E and Q within 1e-9 relative; fp32 runs within 1e-4
+relative energy of the fp64 oracle.  Relative differences use the floor
+max(|E|, h^2 sum |e_i|) because chiral-magnet energies cross zero during relaxation.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2603_24370_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+CHECKPOINTS = (1, 2, 5, 10, 20, 50, 100)
+
+
+def _ss():
+    from paper_2603_24370_b200 import ss
+    return ss
+
+
+def _model(w, b=0):
+    B = w.B if w.B_batch is None else float(w.B_batch[b])
+    return oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam)
+
+
+def _floor(m, phi, E):
+    _, _, de, _ = oracle.energy_charge(m, phi, densities=True)
+    return max(abs(E), m.h * m.h * float(np.abs(de).sum()), 1e-300)
+
+
+def _dev(a, dtype=torch.float64):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0", dtype=dtype).contiguous()
+
+
+def _run_parity(w, checkpoints=CHECKPOINTS, flags=0, field_tol=1e-11, lattices=None):
+    ss = _ss()
+    s = ss.solver_for(w, flags=flags)
+    s.set_fields(_dev(w.fields))
+    lattices = range(w.batch) if lattices is None else lattices
+    flows = {}
+    for b in lattices:
+        fl = oracle.Flow(_model(w, b), w.dt)
+        fl.set_fields(w.fields[b])
+        flows[b] = fl
+    E0 = s.energy()
+    Q0 = s.charge()
+    for b, fl in flows.items():
+        fl0 = _floor(fl.m, w.fields[b], fl.energy)
+        assert abs(E0[b] - fl.energy) <= 1e-12 * fl0
+        assert abs(Q0[b] - fl.charge) <= 1e-12 * max(1.0, abs(fl.charge))
+    done = 0
+    for cp in checkpoints:
+        s.step(cp - done)
+        phi, vel = s.get_fields()
+        E, Q, KE = s.energy(), s.charge(), s.kinetic()
+        phi, vel = phi.cpu().numpy(), vel.cpu().numpy()
+        for b, fl in flows.items():
+            fl.step(cp - done)
+            ophi, ovel = fl.get_fields()
+            assert np.abs(phi[b] - ophi).max() <= field_tol, (cp, b)
+            assert np.abs(vel[b] - ovel).max() <= 10 * field_tol, (cp, b)
+            sc = fl.scalars()
+            fl_ = _floor(fl.m, ophi, sc["E"])
+            assert abs(E[b] - sc["E"]) <= 1e-9 * fl_, (cp, b)
+            assert abs(Q[b] - sc["Q"]) <= 1e-9 * max(1.0, abs(sc["Q"])), (cp, b)
+            assert abs(KE[b] - sc["KE"]) <= 1e-9 * max(fl_, sc["KE"]), (cp, b)
+            got, cnt = s.arrests(b)
+            assert got == fl.arrests() and cnt == sc["n_arrests"], (cp, b)
+        done = cp
+    assert s.status()["steps"] == done
+    return s, flows
+
+
+def test_config1_cm_64_first_100_steps_and_final():
+    w = W.baseline_config(1)
+    s, flows = _run_parity(w)
+    fl = flows[0]
+    s.step(900)
+    fl.step(900)
+    phi = s.get_fields(want_vel=False).cpu().numpy()[0]
+    E, Q = s.energy()[0], s.charge()[0]
+    assert abs(E - fl.energy) <= 1e-9 * _floor(fl.m, phi, fl.energy)
+    assert abs(Q - fl.charge) <= 1e-9 * abs(fl.charge)
+    # after convergence late arrest decisions are rounding noise: fields agree only to ~sqrt(eps)
+    assert np.abs(phi - fl.get_fields()[0]).max() <= 1e-5
+    assert np.abs((phi * phi).sum(0) - 1.0).max() < 1e-14
+
+
+def test_cm_multi_ragged_tiles():
+    # config 2 recipe on a lattice that is not a multiple of the tile (ragged tail in x and y)
+    w = W.cm_multi(N=250, count=3, margin=12.0, min_sep=14.0)
+    _run_parity(w)
+
+
+def test_cm_quench_with_anisotropy():
+    # config 4 recipe (random unit vectors, K = 0.3), several tiles
+    w = W.cm_quench(N=192)
+    _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50))
+
+
+def test_ah_vortices_lambda_1_and_2():
+    for lam in (1.0, 2.0):
+        w = W.ah_vortices(N=150, h=0.1, lam=lam, count=2, min_sep=2.0)
+        _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50))
+
+
+def test_batched_sweep_per_lattice_arrests():
+    w = W.cm_sweep(batch=6, N=96)
+    s, flows = _run_parity(w)
+    logs = [tuple(s.arrests(b)[0]) for b in range(w.batch)]
+    assert len(set(logs)) > 1            # different B -> different arrest histories
+
+
+def test_graph_and_direct_launch_agree_bitwise():
+    ss = _ss()
+    w = W.cm_single(N=96)
+    outs = []
+    for flags in (0, ss.FLAG_NO_GRAPH):
+        s = ss.solver_for(w, flags=flags)
+        s.set_fields(_dev(w.fields))
+        s.step(37)
+        f, v = s.get_fields()
+        outs.append((f.cpu(), v.cpu(), s.energy(), s.charge(), s.arrests(0)))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    assert outs[0][2:] == outs[1][2:]
+
+
+def test_fp32_energy_within_1e4_of_fp64_oracle():
+    ss = _ss()
+    w = W.cm_single(N=64)
+    s = ss.solver_for(w, dtype=ss.F32)
+    s.set_fields(_dev(w.fields, torch.float32))
+    fl = oracle.Flow(_model(w), w.dt)
+    fl.set_fields(w.fields[0])
+    for _ in range(5):
+        s.step(100)
+        fl.step(100)
+        phi = fl.get_fields()[0]
+        assert abs(s.energy()[0] - fl.energy) <= 1e-4 * _floor(fl.m, phi, fl.energy)
+    assert abs(s.charge()[0] - fl.charge) < 1e-4
+
+
+def test_checkpoint_roundtrip_is_bit_exact():
+    ss = _ss()
+    w = W.cm_single(N=80)
+    a = ss.solver_for(w)
+    a.set_fields(_dev(w.fields))
+    a.step(9)
+    assert a.status()["n_arrests"] == [0]
+    f, v = a.get_fields()
+    b = ss.solver_for(w)
+    b.set_fields(f, v)
+    f2, v2 = b.get_fields()
+    assert torch.equal(f, f2) and torch.equal(v, v2)
+    assert b.energy() == a.energy() and b.charge() == a.charge()
+    a.step(5)
+    b.step(5)
+    assert torch.equal(a.get_fields()[0], b.get_fields()[0])
+    # halo is frozen; halo velocities read as zero
+    mask = torch.from_numpy(~W.interior_mask(80, 80)).to("cuda:0")
+    fa, va = a.get_fields()
+    assert torch.equal(fa[0][:, mask], _dev(w.fields)[0][:, mask])
+    assert float(va[0][:, mask].abs().max()) == 0.0
+
+
+def test_smallest_lattices_and_vacuum():
+    ss = _ss()
+    for Nx, Ny in ((6, 5), (6, 6), (8, 7)):
+        rng = np.random.default_rng(Nx * 10 + Ny)
+        f = rng.standard_normal((1, 3, Ny, Nx))
+        f /= np.sqrt((f * f).sum(1, keepdims=True))
+        w = W.Workload("tiny", W.CM, Nx, Ny, 0.2, 0.1, kappa=1.0, B=0.6, K=0.1, fields=f)
+        _run_parity(w, checkpoints=(1, 2, 5))
+    vac = np.zeros((1, 3, 40, 70))
+    vac[0, 2] = 1.0
+    w = W.Workload("vac", W.CM, 70, 40, 0.2, 0.1, kappa=1.0, B=0.6, K=0.3, fields=vac)
+    s = ss.solver_for(w)
+    s.set_fields(_dev(vac))
+    s.step(3)
+    assert s.energy() == [0.0] and s.charge() == [0.0] and s.kinetic() == [0.0]
+    assert torch.equal(s.get_fields(want_vel=False).cpu(), torch.from_numpy(vac))
+
+
+def test_error_paths():
+    ss = _ss()
+    with pytest.raises(ss.SSError) as e:
+        ss.Solver(0, 63, 64, 0.2)                      # odd Nx in fp64
+    assert e.value.code == ss.ERR_ARG
+    with pytest.raises(ss.SSError):
+        ss.Solver(7, 64, 64, 0.2)                      # unknown theory
+    s = ss.Solver(0, 64, 64, 0.2, kappa=1.0, B=0.6)
+    with pytest.raises(ss.SSError) as e:
+        s.step(1)                                      # before set_fields
+    assert e.value.code == ss.ERR_STATE
+    bad = np.full((1, 3, 64, 64), np.nan)
+    s.set_fields(_dev(bad))
+    with pytest.raises(ss.SSError) as e:
+        s.energy()
+    assert e.value.code == ss.ERR_NONFINITE
+    assert math.isnan(s.energy(strict=False)[0])
