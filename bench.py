@@ -1,0 +1,393 @@
+#!/usr/bin/env python
+"""Benchmark of the arrested-Newton-flow hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+A "step" is one flow step n -> n+1 of the whole hot path (RK4 stages 2-4 + update + projection,
+then the stencil pass a1/E/Q on the new field, the tree reductions and the device-side arrest):
+exactly what ss_step(1) enqueues.  Default workload: BASELINE.json configs[3] in fp64 (chiral
+magnet 4096x4096, K = 0.3, random unit vectors) -- the configuration the metric's HBM-roofline
+target is quoted on.  Inputs are seeded and synthetic (paper_2603_24370_b200/workloads.py).
+
+One JSON line on stdout (rank 0).  `value` is whole-job lattice site-updates/s with the state
+resident in HBM; `e2e` is the same metric through the C-ABI host-buffer calls
+(ss_set_fields_host -> ss_step -> ss_energy/ss_charge -> ss_get_fields_host) with every copy
+inside the timed region; `roofline` is the dominant kernel's algorithmic bytes over its
+CUDA-event time (ss_profile_step) against the measured copy bandwidth; `cpu_baseline` is the
+CPU oracle timed on this box's host cores on a bounded sample of the same workload.
+
+--impl reference times the oracle itself (the only reference this paper has: it ships no code).
+N > 1 (torchrun): the path is "replicas only" -- every rank advances its
+own lattice, no data-path collective; time = max over ranks; value = sum of site-updates / time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "lattice site-updates/s per flow step"
+UNIT = "site-updates/s"
+
+# name -> (workloads factory name, kwargs, dtype name)
+WORKLOADS = {
+    "cm4096_f64": ("cm_quench", {}, "f64"),            # BASELINE configs[3], fp64 (default)
+    "cm4096_f32": ("cm_quench", {}, "f32"),            # BASELINE configs[3], fp32
+    "cm1024_f64": ("cm_multi", {}, "f64"),             # BASELINE configs[1] (fits in L2: context)
+    "ah2048_f64": ("ah_vortices", {}, "f64"),          # BASELINE configs[2], lambda = 1
+    "sweep256_f64": ("cm_sweep", {}, "f64"),           # BASELINE configs[4], 256 lattices
+    "cm64_f64": ("cm_single", {}, "f64"),              # BASELINE configs[0] (launch-bound)
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--workload", default="cm4096_f64", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=20.0,
+                    help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def make_workload(name):
+    from paper_2603_24370_b200 import workloads as W
+    fn, kw, dt = WORKLOADS[name]
+    return getattr(W, fn)(**kw), dt
+
+
+def peaks():
+    """Measured HBM copy bandwidth (driver-written), else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    def __init__(self, index, period=0.1):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+            nv.nvmlClocksThrottleReasonApplicationsClocksSetting: "applications_clocks",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def nvml_index(torch, dev):
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+        h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+        return pynvml.nvmlDeviceGetIndex(h)
+    except Exception:
+        return dev.index or 0
+
+
+def time_oracle(w, seconds, lattices=None):
+    """Oracle as it stands on this box's host cores: one untimed step, then as many steps as fit
+    in about `seconds` (at least 1) on lattice 0 (and only lattice 0 of a batched workload)."""
+    import oracle
+    b = 0
+    B = w.B if w.B_batch is None else float(w.B_batch[b])
+    fl = oracle.Flow(oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K,
+                                  lam=w.lam), w.dt)
+    fl.set_fields(w.fields[b])
+    t0 = time.perf_counter()
+    fl.step(1)
+    t1 = time.perf_counter() - t0
+    k = max(1, min(1000, int(seconds / max(t1, 1e-6)) - 1))
+    t0 = time.perf_counter()
+    fl.step(k)
+    t = time.perf_counter() - t0
+    sites = (w.Nx - 4) * (w.Ny - 4)
+    return {"value": sites * k / t, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"{k} flow steps of lattice 0 of {w.name} ({w.Nx}x{w.Ny}, fp64, full "
+                      f"size) after 1 untimed step; {t:.1f} s",
+            "ms_per_step": 1e3 * t / k, "steps": k}
+
+
+def crop_workload(w, S):
+    """Top-left S x S window of lattice 0 (its outer two rings become the frozen halo)."""
+    import copy
+    c = copy.copy(w)
+    c.Nx = c.Ny = S
+    c.batch = 1
+    c.fields = w.fields[:1, :, :S, :S].copy()
+    c.B = w.B if w.B_batch is None else float(w.B_batch[0])
+    c.B_batch = None
+    c.name = f"{w.name}[crop {S}x{S}]"
+    return c
+
+
+def run_reference(args):
+    """--impl reference: the paper ships no code, so the reference arm is the CPU oracle, as it
+    stands, on this box's host cores.  Each of the W + K steps is one oracle flow step on a
+    bounded sample of the workload: a square crop sized (from one calibration step on a 256^2
+    crop) so that the whole run takes about two minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w, _ = make_workload(args.workload)
+    full = min(w.Nx, w.Ny)
+    cal = crop_workload(w, min(256, full))
+    rate = time_oracle(cal, 0.0)["value"]                     # site-updates/s, 1 step
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    S = int((rate * budget) ** 0.5) // 64 * 64
+    S = max(64, min(full, S))
+    c = crop_workload(w, S)
+    fl = oracle.Flow(oracle.model(c.theory, S, S, c.h, kappa=c.kappa, B=c.B, K=c.K, lam=c.lam),
+                     c.dt)
+    fl.set_fields(c.fields[0])
+    fl.step(args.warmup)
+    t0 = time.perf_counter()
+    fl.step(args.steps)
+    t = time.perf_counter() - t0
+    value = (S - 4) * (S - 4) * args.steps / t
+    cpu = {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+           "sample": f"{args.steps} flow steps (after {args.warmup} warm-up) of the top-left "
+                     f"{S}x{S} crop of {w.name}, fp64; {t:.1f} s"}
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded)",
+        "config": {"workload": w.name, "sample": f"crop {S}x{S}", "theory":
+                   "chiral_magnet" if w.theory == 0 else "abelian_higgs", "h": w.h, "dt": w.dt},
+        "cpu_baseline": cpu,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# Algorithmic bytes per interior site of each kernel of one flow step, in units of C*sizeof(real)
+# (DESIGN.md "Kernels and traffic model"): what the kernel must read + write once.
+KERNEL_UNITS = {
+    "stage2": 3,                       # reads phi, v            -> writes a2
+    "stage3": 4,                       # reads phi, v, a1        -> writes a3
+    "stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
+    "stage1_grad_energy_charge": 2,    # reads phi'              -> writes a1 (+ E, Q partials)
+}
+STEP_UNITS_OURS = sum(KERNEL_UNITS.values())   # 16
+STEP_UNITS_SURVEY = 21                          # stage fields materialised
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2603_24370_b200 import ss      # raises if libss.so is missing: no CPU fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (libss has no CPU path)")
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w, dtname = make_workload(args.workload)
+    dtype = ss.F64 if dtname == "f64" else ss.F32
+    tdt = torch.float64 if dtname == "f64" else torch.float32
+    R = 8 if dtname == "f64" else 4
+    host = torch.from_numpy(w.fields).to(tdt).contiguous().pin_memory()
+    s = ss.solver_for(w, dtype=dtype, device=str(dev))
+    s.set_fields(host.to(dev))
+    sites = w.interior_sites
+    field_bytes = host.numel() * R
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K steps
+    s.step(args.warmup)
+    barrier()
+    n0 = s.launch_count()
+    sampler = ClockSampler(nvml_index(torch, dev))
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    s.step(args.steps)
+    e1.record(s.stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = s.launch_count() - n0
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * sites * args.steps / (ms * 1e-3)
+    st = s.status()
+
+    # ---- per-kernel CUDA-event times of the same step (kernels launched one by one)
+    prof = s.profile_step(reps=min(20, max(3, args.steps)))
+    peak, peak_src = peaks()
+    C = w.C
+    kern = {}
+    for name, kms in prof:
+        u = KERNEL_UNITS.get(name)
+        kern[name] = {"ms": kms}
+        if u:
+            kern[name]["alg_bytes"] = u * C * R * sites
+            kern[name]["gbs"] = u * C * R * sites / (kms * 1e-3) / 1e9
+    dom = max((n for n in kern if "gbs" in kern[n]), key=lambda n: kern[n]["ms"])
+    tot = sum(k["ms"] for k in kern.values())
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
+        "unit": "GB/s", "frac": kern[dom]["gbs"] / peak, "traffic": None,
+        "peak_source": peak_src, "kernel_ms": kern[dom]["ms"],
+        "kernel_share_of_step": kern[dom]["ms"] / tot,
+        "alg_bytes_per_site": KERNEL_UNITS[dom] * C * R,
+        "step": {
+            "ms_graph": ms / args.steps,
+            "ms_sum_of_kernels": tot,
+            "gbs_schedule_16CR": STEP_UNITS_OURS * C * R * sites * args.steps / (ms * 1e-3) / 1e9,
+            "gbs_survey_21CR": STEP_UNITS_SURVEY * C * R * sites * args.steps / (ms * 1e-3) / 1e9,
+            "frac_of_peak_16CR": STEP_UNITS_OURS * C * R * sites * args.steps / (ms * 1e-3) / 1e9 / peak,
+            "frac_of_8TBs_21CR": STEP_UNITS_SURVEY * C * R * sites * args.steps / (ms * 1e-3) / 1e9 / 8000.0,
+        },
+        "kernels": kern,
+    }
+    return dict(torch=torch, dist=dist, s=s, w=w, host=host, dev=dev, rank=rank, world=world,
+                value=value, ms=ms, launches=launches, clocks=clocks, roofline=roofline,
+                status=st, sites=sites, field_bytes=field_bytes, dtname=dtname, barrier=barrier)
+
+
+def run_e2e(r, args):
+    """Same metric through the host-buffer C-ABI calls, every copy inside the timed region:
+    pinned host fields -> ss_set_fields_host -> ss_step(K) -> ss_energy + ss_charge (D2H) ->
+    ss_get_fields_host (fields back to pinned host memory).  The flow's state is device-resident
+    by construction ("device buffers"), so one job pays the copies once per K steps;
+    `roundtrip_every_step` is the worst case where a user uploads and downloads around every
+    single step."""
+    torch, s, host, dev = r["torch"], r["s"], r["host"], r["dev"]
+    out = torch.empty_like(host).pin_memory()
+    K = args.steps
+
+    def job(k):
+        r["barrier"]()
+        t0 = time.perf_counter()
+        s.set_fields_host(host)
+        s.step(k)
+        E = s.energy(strict=False)
+        Q = s.charge(strict=False)
+        s.get_fields_host(out)
+        torch.cuda.synchronize(dev)
+        return time.perf_counter() - t0, E, Q
+
+    job(min(K, 3))                                        # warm the pinned paths
+    t, E, Q = job(K)
+    trt = min(job(1)[0] for _ in range(3))
+    if r["world"] > 1:
+        tt = torch.tensor([t, trt], device=dev, dtype=torch.float64)
+        r["dist"].all_reduce(tt, op=r["dist"].ReduceOp.MAX)
+        t, trt = float(tt[0]), float(tt[1])
+    nsc = 2 * 8 * r["w"].batch
+    return {
+        "value": r["world"] * r["sites"] * K / t, "unit": UNIT,
+        "h2d_bytes_per_step": r["field_bytes"] / K,
+        "d2h_bytes_per_step": (r["field_bytes"] + nsc) / K,
+        "job": f"set_fields_host + {K} steps + energy/charge + get_fields_host, {t * 1e3:.1f} ms",
+        "roundtrip_every_step": {"value": r["world"] * r["sites"] / trt, "unit": UNIT,
+                                 "h2d_bytes_per_step": r["field_bytes"],
+                                 "d2h_bytes_per_step": r["field_bytes"] + nsc,
+                                 "ms_per_step": trt * 1e3},
+        "E": E[0], "Q": Q[0],
+    }
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    r = run_ours(args)
+    e2e = run_e2e(r, args)
+    w = r["w"]
+    cpu = None
+    if r["rank"] == 0 and r["world"] == 1 and not args.no_cpu_baseline:
+        cpu = time_oracle(w, args.cpu_seconds)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"} & set(r["clocks"]["reasons"])
+    line = {
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": r["world"],
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms"] / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": r["dtname"], "data": "synthetic (seeded)",
+        "config": {"workload": w.name, "theory": "chiral_magnet" if w.theory == 0 else
+                   "abelian_higgs", "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
+                   "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
+                   "integrator": "rk4", "parallelism": f"replicas x{r['world']}",
+                   "l2_policy": "working set (7 field arrays) larger than L2; no flush needed"
+                   if 7 * r["field_bytes"] > 3 * 126e6 else
+                   "working set comparable to L2: not roofline evidence"},
+        "e2e": e2e, "gpu_launches": r["launches"], "clocks": r["clocks"],
+        "clocks_rejected": sorted(bad),
+        "roofline": r["roofline"], "cpu_baseline": cpu,
+        "state": {"steps_done": r["status"]["steps"], "n_arrests": r["status"]["n_arrests"][:4]},
+    }
+    if r["rank"] == 0:
+        print(json.dumps(line), flush=True)
+    if r["world"] > 1:
+        r["dist"].destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

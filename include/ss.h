@@ -98,6 +98,12 @@ int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev);
  * the velocity reads as exactly 0. */
 int ss_get_fields(ss_solver* s, void* fields_dev, void* vel_dev);
 
+/* The same two calls for HOST arrays (same layout and semantics; pinned memory makes the
+ * copies asynchronous).  The transfers go straight to / from the workspace on the stream;
+ * ss_get_fields_host synchronises the stream before returning. */
+int ss_set_fields_host(ss_solver* s, const void* fields_host, const void* vel_host);
+int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
+
 /* Enqueue k flow steps (asynchronous; no host synchronisation, the arrest of eq. 4 is
  * decided on the device).  One step = RK4 stages 2-4 + update + projection, then the
  * stencil pass on the new field (a, E, Q) and the arrest decision. */
@@ -117,6 +123,14 @@ int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int6
 
 /* Number of kernel launches (graph nodes included) enqueued by this handle so far. */
 int64_t ss_launch_count(const ss_solver* s);
+
+/* Measurement aid: run `reps` real flow steps launching the step's kernels one by one with a
+ * CUDA event between consecutive launches on the solver's stream, and return the average
+ * device time of each kernel in milliseconds (HOST array, `cap` entries; *n_kernels = number
+ * of kernels in one step, in launch order; ss_kernel_name(i) names entry i).  The state
+ * advances by `reps` steps exactly as with ss_step(reps).  Synchronises the stream. */
+int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_kernels);
+const char* ss_kernel_name(const ss_solver* s, int i);
 
 const char* ss_strerror(int code);
 

@@ -66,6 +66,7 @@ def lib():
                                        C.POINTER(C.c_int)]
         L.orc_flow_arrests.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int64]
         L.orc_flow_arrests.restype = C.c_int64
+        L.orc_threads.restype = C.c_int
         _lib = L
     return _lib
 
@@ -77,6 +78,11 @@ def _p(a):
 def _f64(a):
     a = np.ascontiguousarray(a, dtype=np.float64)
     return a
+
+
+def threads() -> int:
+    """OpenMP threads the oracle's loops run on."""
+    return int(lib().orc_threads())
 
 
 def ncomp(theory: int) -> int:

@@ -27,6 +27,7 @@
  *   (DESIGN R7) has no external pin beyond those order/invariant checks.
  */
 #include <math.h>
+#include <omp.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -617,3 +618,6 @@ int64_t orc_flow_arrests(const orc_flow* s, int64_t* out, int64_t cap) {
   memcpy(out, s->log, c * sizeof(int64_t));
   return s->nlog;
 }
+
+/* number of OpenMP threads the parallel loops above use (reported by bench.py) */
+int orc_threads(void) { return omp_get_max_threads(); }

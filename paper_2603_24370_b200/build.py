@@ -30,6 +30,14 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def declared_symbols():
+    """Names of the functions include/ss.h declares (every one must be exported by libss.so)."""
+    import re
+    text = open(os.path.join(HERE, "..", "include", "ss.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ss_[a-z_]+)\s*\(", text)))
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources()

@@ -82,6 +82,7 @@ struct KernelNode {
   dim3 grid, block;
   size_t smem;
   std::vector<unsigned char> args;  // the single by-value argument struct
+  const char* name;
 };
 
 template <int THEORY, typename real>
@@ -165,6 +166,9 @@ KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
   n.block = dim3(BX, BY, 1);
   n.smem = (size_t)s->C * TYP * TXP * sizeof(real);
   n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  static const char* names[4] = {"stage1_grad_energy_charge", "stage2", "stage3",
+                                 "stage4_combine_project_ke"};
+  n.name = names[stage - 1];
   return n;
 }
 
@@ -191,8 +195,10 @@ void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>&
   r.block = dim3(256, 1, 1);
   r.smem = 0;
   r.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  r.name = "row_reduce";
   out.push_back(r);
   KernelNode f = r;
+  f.name = "finalize_arrest";
   f.func = (void*)finalize_kernel;
   f.grid = dim3(s->batch, 1, 1);
   f.block = dim3(1024, 1, 1);
@@ -321,23 +327,31 @@ int ss_destroy(ss_solver* s) {
   return SS_OK;
 }
 
-int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev) {
-  if (!s || !fields_dev) return SS_ERR_ARG;
+// fields go to phi(0) and phi(1); velocities are staged in vel(1) (host source) or read from
+// the caller's array (device source) and masked to the interior into vel(0).
+static int set_fields_impl(ss_solver* s, const void* fields, const void* vel, cudaMemcpyKind kind) {
+  if (!s || !fields) return SS_ERR_ARG;
   const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
   const long long planes = (long long)s->batch * s->C;
-  CK(cudaMemcpyAsync(s->phi(0), fields_dev, nbytes, cudaMemcpyDeviceToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->phi(1), fields_dev, nbytes, cudaMemcpyDeviceToDevice, s->stream));
-  CK(cudaMemsetAsync(s->vel(0), 0, nbytes, s->stream));
-  CK(cudaMemsetAsync(s->vel(1), 0, nbytes, s->stream));
-  if (vel_dev) {
+  CK(cudaMemcpyAsync(s->phi(0), fields, nbytes, kind, s->stream));
+  CK(cudaMemcpyAsync(s->phi(1), s->phi(0), nbytes, cudaMemcpyDeviceToDevice, s->stream));
+  const void* vsrc = vel;
+  if (vel && kind == cudaMemcpyHostToDevice) {
+    CK(cudaMemcpyAsync(s->vel(1), vel, nbytes, kind, s->stream));
+    vsrc = s->vel(1);
+  }
+  if (vsrc) {
     if (s->dtype == SS_F64)
-      copy_interior_kernel<double><<<1184, 256, 0, s->stream>>>((double*)s->vel(0), (const double*)vel_dev,
+      copy_interior_kernel<double><<<1184, 256, 0, s->stream>>>((double*)s->vel(0), (const double*)vsrc,
                                                                  s->Nx, s->Ny, planes);
     else
-      copy_interior_kernel<float><<<1184, 256, 0, s->stream>>>((float*)s->vel(0), (const float*)vel_dev,
+      copy_interior_kernel<float><<<1184, 256, 0, s->stream>>>((float*)s->vel(0), (const float*)vsrc,
                                                                 s->Nx, s->Ny, planes);
     s->launches += 1;
+  } else {
+    CK(cudaMemsetAsync(s->vel(0), 0, nbytes, s->stream));
   }
+  CK(cudaMemsetAsync(s->vel(1), 0, nbytes, s->stream));
   for (int i = 0; i < 3; ++i) CK(cudaMemsetAsync(s->part(i), 0, s->L.part_bytes, s->stream));
   init_state_kernel<<<(s->batch + 127) / 128, 128, 0, s->stream>>>(s->state(), s->batch);
   s->launches += 1;
@@ -348,24 +362,43 @@ int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev) {
   return launch_nodes(s, s->eval_nodes[0]);
 }
 
-int ss_get_fields(ss_solver* s, void* fields_dev, void* vel_dev) {
+int ss_set_fields(ss_solver* s, const void* fields_dev, const void* vel_dev) {
+  return set_fields_impl(s, fields_dev, vel_dev, cudaMemcpyDeviceToDevice);
+}
+int ss_set_fields_host(ss_solver* s, const void* fields_host, const void* vel_host) {
+  return set_fields_impl(s, fields_host, vel_host, cudaMemcpyHostToDevice);
+}
+
+// velocities are exported (zero when the last step was arrested) either into the
+// caller's device array or, for a host destination, into the idle ping-pong velocity buffer,
+// which the next step overwrites on the interior and never reads.
+static int get_fields_impl(ss_solver* s, void* fields, void* vel, cudaMemcpyKind kind) {
   if (!s) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
   const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
-  if (fields_dev)
-    CK(cudaMemcpyAsync(fields_dev, s->phi(s->cur), nbytes, cudaMemcpyDeviceToDevice, s->stream));
-  if (vel_dev) {
+  if (fields) CK(cudaMemcpyAsync(fields, s->phi(s->cur), nbytes, kind, s->stream));
+  if (vel) {
     const long long per = (long long)s->C * s->Ny * s->Nx;
+    void* dst = kind == cudaMemcpyDeviceToHost ? s->vel(s->cur ^ 1) : vel;
     if (s->dtype == SS_F64)
       export_velocity_kernel<double><<<1184, 256, 0, s->stream>>>(
-          (double*)vel_dev, (const double*)s->vel(s->cur), s->state(), per, s->batch);
+          (double*)dst, (const double*)s->vel(s->cur), s->state(), per, s->batch);
     else
       export_velocity_kernel<float><<<1184, 256, 0, s->stream>>>(
-          (float*)vel_dev, (const float*)s->vel(s->cur), s->state(), per, s->batch);
+          (float*)dst, (const float*)s->vel(s->cur), s->state(), per, s->batch);
     s->launches += 1;
     CK(cudaGetLastError());
+    if (kind == cudaMemcpyDeviceToHost) CK(cudaMemcpyAsync(vel, dst, nbytes, kind, s->stream));
   }
+  if (kind == cudaMemcpyDeviceToHost) CK(cudaStreamSynchronize(s->stream));
   return SS_OK;
+}
+
+int ss_get_fields(ss_solver* s, void* fields_dev, void* vel_dev) {
+  return get_fields_impl(s, fields_dev, vel_dev, cudaMemcpyDeviceToDevice);
+}
+int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host) {
+  return get_fields_impl(s, fields_host, vel_host, cudaMemcpyDeviceToHost);
 }
 
 int ss_step(ss_solver* s, int64_t k) {
@@ -434,6 +467,46 @@ int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int6
     CK(cudaStreamSynchronize(s->stream));
   }
   return SS_OK;
+}
+
+int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_kernels) {
+  if (!s || !ms_host || !n_kernels || reps < 1) return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  const int n = (int)s->step_nodes[0].size();
+  *n_kernels = n;
+  if (cap < n) return SS_ERR_ARG;
+  std::vector<cudaEvent_t> ev(n + 1);
+  for (auto& e : ev) CK(cudaEventCreate(&e));
+  std::vector<double> acc(n, 0.0);
+  int rc = SS_OK;
+  for (int it = 0; it < reps && rc == SS_OK; ++it) {
+    auto& nodes = s->step_nodes[s->cur];
+    cudaError_t e = cudaEventRecord(ev[0], s->stream);
+    for (int i = 0; i < n && e == cudaSuccess; ++i) {
+      void* params[1] = {nodes[i].args.data()};
+      e = cudaLaunchKernel(nodes[i].func, nodes[i].grid, nodes[i].block, params, nodes[i].smem,
+                           s->stream);
+      if (e == cudaSuccess) e = cudaEventRecord(ev[i + 1], s->stream);
+      s->launches += 1;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    for (int i = 0; i < n && e == cudaSuccess; ++i) {
+      float ms = 0.f;
+      e = cudaEventElapsedTime(&ms, ev[i], ev[i + 1]);
+      acc[i] += ms;
+    }
+    if (!cuda_ok(e, "ss_profile_step")) rc = SS_ERR_CUDA;
+    s->cur ^= 1;
+    s->steps_done += 1;
+  }
+  for (auto& e : ev) cudaEventDestroy(e);
+  for (int i = 0; i < n; ++i) ms_host[i] = acc[i] / reps;
+  return rc;
+}
+
+const char* ss_kernel_name(const ss_solver* s, int i) {
+  if (!s || i < 0 || i >= (int)s->step_nodes[0].size()) return "";
+  return s->step_nodes[0][i].name;
 }
 
 int64_t ss_launch_count(const ss_solver* s) { return s ? s->launches : 0; }

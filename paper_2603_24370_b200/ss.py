@@ -26,6 +26,7 @@ OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE 
 FLAG_NO_GRAPH = 1
 
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
+           "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",
            "ss_step", "ss_energy", "ss_charge", "ss_kinetic", "ss_status", "ss_arrests",
            "ss_launch_count", "ss_strerror"]
 
@@ -47,6 +48,11 @@ _lib.ss_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c
 _lib.ss_destroy.argtypes = [C.c_void_p]
 _lib.ss_set_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ss_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.ss_set_fields_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.ss_get_fields_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.ss_profile_step.argtypes = [C.c_void_p, C.c_int, _dp, C.c_int, C.POINTER(C.c_int)]
+_lib.ss_kernel_name.argtypes = [C.c_void_p, C.c_int]
+_lib.ss_kernel_name.restype = C.c_char_p
 _lib.ss_step.argtypes = [C.c_void_p, C.c_int64]
 for _n in ("ss_energy", "ss_charge", "ss_kinetic"):
     getattr(_lib, _n).argtypes = [C.c_void_p, _dp]
@@ -154,8 +160,34 @@ class Solver:
                    "ss_get_fields")
         return (f, v) if want_vel else f
 
+    def _host(self, t, name):
+        if t is None:
+            return None
+        if not (not t.is_cuda and t.dtype == self.torch_dtype and t.is_contiguous()
+                and tuple(t.shape) == self.shape):
+            raise ValueError(f"{name}: need a contiguous {self.torch_dtype} CPU tensor of shape "
+                             f"{self.shape}")
+        return C.c_void_p(t.data_ptr())
+
+    def set_fields_host(self, fields, vel=None):
+        """fields / vel: CPU tensors (pinned for asynchronous copies)."""
+        _check(_lib.ss_set_fields_host(self._h, self._host(fields, "fields"),
+                                       self._host(vel, "vel")), "ss_set_fields_host")
+
+    def get_fields_host(self, fields=None, vel=None):
+        """Fill the given CPU tensors (either may be None); synchronises the stream."""
+        _check(_lib.ss_get_fields_host(self._h, self._host(fields, "fields"),
+                                       self._host(vel, "vel")), "ss_get_fields_host")
+
     def step(self, k=1):
         _check(_lib.ss_step(self._h, int(k)), "ss_step")
+
+    def profile_step(self, reps=1):
+        """[(kernel name, average ms)] of one flow step, kernels launched one by one."""
+        buf = (C.c_double * 16)()
+        n = C.c_int()
+        _check(_lib.ss_profile_step(self._h, int(reps), buf, 16, C.byref(n)), "ss_profile_step")
+        return [(_lib.ss_kernel_name(self._h, i).decode(), buf[i]) for i in range(n.value)]
 
     def _scalar(self, fn, name, strict):
         out = (C.c_double * self.batch)()
