@@ -55,6 +55,8 @@ def parse_args():
     ap.add_argument("--workload", default="cm4096_f64", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--staged", action="store_true", help="one kernel per RK4 stage (A/B)")
+    ap.add_argument("--cps", type=int, default=0, help="chunks per segment (0 = auto)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0,
                     help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -215,12 +217,15 @@ def run_reference(args):
 # Algorithmic bytes per interior site of each kernel of one flow step, in units of C*sizeof(real)
 # (DESIGN.md "Kernels and traffic model"): what the kernel must read + write once.
 KERNEL_UNITS = {
+    # two-kernel schedule (default)
+    "flow_y_stage34_combine_project_ke": 6,   # reads phi, v, a1, a2 -> writes phi', v'
+    "flow_x_grad_energy_charge_stage2": 4,    # reads phi', v'       -> writes a1, a2 (+ E, Q partials)
+    # one kernel per RK4 stage (--staged, the first round-1 schedule)
     "stage2": 3,                       # reads phi, v            -> writes a2
     "stage3": 4,                       # reads phi, v, a1        -> writes a3
     "stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
     "stage1_grad_energy_charge": 2,    # reads phi'              -> writes a1 (+ E, Q partials)
 }
-STEP_UNITS_OURS = sum(KERNEL_UNITS.values())   # 16
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
 
@@ -245,7 +250,8 @@ def run_ours(args):
     tdt = torch.float64 if dtname == "f64" else torch.float32
     R = 8 if dtname == "f64" else 4
     host = torch.from_numpy(w.fields).to(tdt).contiguous().pin_memory()
-    s = ss.solver_for(w, dtype=dtype, device=str(dev))
+    s = ss.solver_for(w, dtype=dtype, device=str(dev), cps=args.cps,
+                      flags=ss.FLAG_STAGED if args.staged else 0)
     s.set_fields(host.to(dev))
     sites = w.interior_sites
     field_bytes = host.numel() * R
@@ -289,6 +295,7 @@ def run_ours(args):
             kern[name]["gbs"] = u * C * R * sites / (kms * 1e-3) / 1e9
     dom = max((n for n in kern if "gbs" in kern[n]), key=lambda n: kern[n]["ms"])
     tot = sum(k["ms"] for k in kern.values())
+    units = sum(KERNEL_UNITS.get(n, 0) for n in kern)      # 10 (two-kernel) or 16 (staged)
     roofline = {
         "bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
         "unit": "GB/s", "frac": kern[dom]["gbs"] / peak, "traffic": None,
@@ -298,9 +305,10 @@ def run_ours(args):
         "step": {
             "ms_graph": ms / args.steps,
             "ms_sum_of_kernels": tot,
-            "gbs_schedule_16CR": STEP_UNITS_OURS * C * R * sites * args.steps / (ms * 1e-3) / 1e9,
+            "schedule_units_of_CR": units,
+            "gbs_schedule": units * C * R * sites * args.steps / (ms * 1e-3) / 1e9,
             "gbs_survey_21CR": STEP_UNITS_SURVEY * C * R * sites * args.steps / (ms * 1e-3) / 1e9,
-            "frac_of_peak_16CR": STEP_UNITS_OURS * C * R * sites * args.steps / (ms * 1e-3) / 1e9 / peak,
+            "frac_of_peak_schedule": units * C * R * sites * args.steps / (ms * 1e-3) / 1e9 / peak,
             "frac_of_8TBs_21CR": STEP_UNITS_SURVEY * C * R * sites * args.steps / (ms * 1e-3) / 1e9 / 8000.0,
         },
         "kernels": kern,
@@ -374,7 +382,8 @@ def main():
         "config": {"workload": w.name, "theory": "chiral_magnet" if w.theory == 0 else
                    "abelian_higgs", "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
                    "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
-                   "integrator": "rk4", "parallelism": f"replicas x{r['world']}",
+                   "integrator": "rk4", "schedule": "staged" if args.staged else "two-kernel",
+                   "parallelism": f"replicas x{r['world']}",
                    "l2_policy": "working set (7 field arrays) larger than L2; no flush needed"
                    if 7 * r["field_bytes"] > 3 * 126e6 else
                    "working set comparable to L2: not roofline evidence"},

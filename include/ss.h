@@ -77,6 +77,9 @@ typedef struct {
   int integrator;          /* SS_RK4                                                        */
   int flags;               /* bit 0: launch kernels one by one instead of replaying the     */
                            /* per-step CUDA graph (debugging; same results)                 */
+                           /* bit 1: one kernel per RK4 stage (the round-1 schedule, kept   */
+                           /* for A/B measurements) instead of the two fused flow kernels   */
+  int chunks_per_segment;  /* tuning: rows/4 each CTA of the flow kernels marches; 0 = auto */
 } ss_params;
 
 /* Bytes of device workspace ss_create needs for this problem; 0 on invalid arguments. */

@@ -11,6 +11,7 @@
 #include <new>
 #include <vector>
 
+#include "ss_flow.cuh"
 #include "ss_kernels.cuh"
 
 using namespace ss;
@@ -113,6 +114,7 @@ struct ss_solver {
   int flags;
   bool fields_set;
   int cur;  // which ping-pong buffer holds (phi, v)
+  int cps;  // chunks per y-segment of the flow kernels
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
@@ -175,6 +177,119 @@ KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
 KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
   return s->dtype == SS_F64 ? make_stage_node<double>(s, stage, cur)
                             : make_stage_node<float>(s, stage, cur);
+}
+
+
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) ==
+            cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// field array [batch*C][Ny][Nx] as a 3-D tensor; box = {FW + 2*XPAD, FR, C} starting 16 bytes
+// left of the strip (XPAD = 2 doubles / 4 floats); zero fill outside
+bool make_tmap(const ss_solver* s, void* base, CUtensorMap* out) {
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc) { snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled unavailable"); return false; }
+  cuuint64_t dims[3] = {(cuuint64_t)s->Nx, (cuuint64_t)s->Ny, (cuuint64_t)s->batch * s->C};
+  cuuint64_t strides[2] = {(cuuint64_t)s->Nx * s->R, (cuuint64_t)s->Nx * s->Ny * s->R};
+  cuuint32_t box[3] = {(cuuint32_t)(FW + 32 / s->R), (cuuint32_t)FR, (cuuint32_t)s->C};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(out, s->dtype == SS_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
+                                           : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                   3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return false;
+  }
+  return true;
+}
+
+template <int THEORY, typename real>
+void* flow_func_t(int kind) {
+  return kind == KX ? (void*)flow_kernel<THEORY, real, KX> : (void*)flow_kernel<THEORY, real, KY>;
+}
+void* flow_func(int theory, int dtype, int kind) {
+  if (theory == SS_THEORY_CHIRAL_MAGNET)
+    return dtype == SS_F64 ? flow_func_t<kCM, double>(kind) : flow_func_t<kCM, float>(kind);
+  return dtype == SS_F64 ? flow_func_t<kAH, double>(kind) : flow_func_t<kAH, float>(kind);
+}
+template <int THEORY, typename real>
+int flow_smem_t(int kind) {
+  return kind == KX ? FlowCfg<THEORY, real, KX>::SMEM : FlowCfg<THEORY, real, KY>::SMEM;
+}
+int flow_smem(int theory, int dtype, int kind) {
+  if (theory == SS_THEORY_CHIRAL_MAGNET)
+    return dtype == SS_F64 ? flow_smem_t<kCM, double>(kind) : flow_smem_t<kCM, float>(kind);
+  return dtype == SS_F64 ? flow_smem_t<kAH, double>(kind) : flow_smem_t<kAH, float>(kind);
+}
+
+// kernel X (kind KX) evaluates the state in buffer `in`; kernel Y advances `in` -> `in ^ 1`
+template <typename real>
+bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
+  FlowArgs<real> a;
+  memset(&a, 0, sizeof(a));
+  const double dt = s->dt, h = s->h;
+  if (!make_tmap(s, s->phi(in), &a.tm[0]) || !make_tmap(s, s->vel(in), &a.tm[1]) ||
+      !make_tmap(s, s->acc(0), &a.tm[2]) || !make_tmap(s, s->acc(1), &a.tm[3]))
+    return false;
+  if (kind == KX) {
+    a.out0 = (real*)s->acc(0); a.out1 = (real*)s->acc(1);
+    a.part0 = s->part(0); a.part1 = s->part(1);
+  } else {
+    a.out0 = (real*)s->phi(in ^ 1); a.out1 = (real*)s->vel(in ^ 1);
+    a.part0 = s->part(2); a.part1 = nullptr;
+  }
+  a.state = s->state();
+  a.Bb = (const double*)(s->ws + s->L.off_bb);
+  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg; a.cps = s->cps;
+  a.plane = (long long)s->Nx * s->Ny;
+  a.hdt = real(0.5 * dt); a.dt = real(dt);
+  a.qdt2 = real(0.25 * (dt * dt)); a.hdt2 = real(0.5 * (dt * dt));
+  a.sdt2 = real((dt * dt) / 6.0); a.sdt = real(dt / 6.0);
+  a.i12h = real(1.0 / (12.0 * h)); a.i12h2 = real(1.0 / (12.0 * h * h));
+  a.kappa = real(s->kappa); a.K = real(s->K); a.lambda = real(s->lambda);
+  KernelNode n;
+  n.func = flow_func(s->theory, s->dtype, kind);
+  const int NC = (s->Ny + FR - 1) / FR;
+  n.grid = dim3(s->L.nseg, (NC + s->cps - 1) / s->cps, s->batch);
+  n.block = dim3(FTHREADS, 1, 1);
+  n.smem = (size_t)flow_smem(s->theory, s->dtype, kind);
+  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  n.name = kind == KX ? "flow_x_grad_energy_charge_stage2" : "flow_y_stage34_combine_project_ke";
+  *out = n;
+  return true;
+}
+bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
+  return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out)
+                            : make_flow_node<float>(s, kind, in, out);
+}
+
+// chunks per segment: minimise (waves of CTAs) x (chunks marched per CTA, warm-up included)
+int choose_cps(int nstrips, int Ny, int batch, int slots) {
+  const int NC = (Ny + FR - 1) / FR;
+  long long best = -1;
+  int best_cps = 1;
+  for (int cps = 1; cps <= NC; ++cps) {
+    const long long items = (long long)nstrips * ((NC + cps - 1) / cps) * batch;
+    const long long waves = (items + slots - 1) / slots;
+    const long long cost = waves * (4 * (cps + 2) + 3);  // + per-CTA prologue
+    if (best < 0 || cost < best) { best = cost; best_cps = cps; }
+  }
+  return best_cps;
 }
 
 void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>& out) {
@@ -294,21 +409,54 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);  // bb is a local
   if (!cuda_ok(e, "upload B_batch")) { delete s; return SS_ERR_CUDA; }
 
-  for (int stage = 1; stage <= 4; ++stage) {
-    void* f = stage_func(theory, p->dtype, stage);
-    e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)((size_t)s->C * TYP * TXP * s->R));
-    if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+  const bool staged = (s->flags & 2) != 0;
+  if (staged) {
+    for (int stage = 1; stage <= 4; ++stage) {
+      void* f = stage_func(theory, p->dtype, stage);
+      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)((size_t)s->C * TYP * TXP * s->R));
+      if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+    }
+  } else {
+    int sms = 148, occ = 1, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    for (int kind = 0; kind < 2; ++kind) {
+      void* f = flow_func(theory, p->dtype, kind);
+      const int smem = flow_smem(theory, p->dtype, kind);
+      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+      if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+      int o = 1;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, FTHREADS, smem);
+      if (!cuda_ok(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor") || o < 1) {
+        delete s; return SS_ERR_CUDA;
+      }
+      if (kind == KY) occ = o;  // segment the lattice for the heavier kernel
+    }
+    s->cps = p->chunks_per_segment > 0 ? p->chunks_per_segment
+                                       : choose_cps(L.nseg, Ny, s->batch, sms * occ);
   }
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
-    st.push_back(make_stage_node(s, 2, cur));
-    st.push_back(make_stage_node(s, 3, cur));
-    st.push_back(make_stage_node(s, 4, cur));
-    st.push_back(make_stage_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
-    make_reduce_nodes(s, 1, st);
     auto& ev = s->eval_nodes[cur];
-    ev.push_back(make_stage_node(s, 1, cur));
+    if (staged) {
+      st.push_back(make_stage_node(s, 2, cur));
+      st.push_back(make_stage_node(s, 3, cur));
+      st.push_back(make_stage_node(s, 4, cur));
+      st.push_back(make_stage_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
+      ev.push_back(make_stage_node(s, 1, cur));
+    } else {
+      KernelNode y, x, x0;
+      if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, KX, cur ^ 1, &x) ||
+          !make_flow_node(s, KX, cur, &x0)) {
+        ss_destroy(s);
+        return SS_ERR_CUDA;
+      }
+      st.push_back(y);
+      st.push_back(x);  // a1, a2, E, Q on the new state
+      ev.push_back(x0);
+    }
+    make_reduce_nodes(s, 1, st);
     make_reduce_nodes(s, 0, ev);
     if (!(s->flags & 1)) {
       int rc = build_graph(s, st, &s->step_exec[cur]);

@@ -62,8 +62,8 @@ struct CM {
   static constexpr int C = 3;
 
   // a = -(G - (G.n) n),  G = -(Lx+Ly) n + 2 kappa (Dy n3, -Dx n3, Dx n2 - Dy n1) - (B + 2K n3) e3
-  template <typename Tile>
-  __device__ __forceinline__ static void accel(const Tile& T, const StageArgs<real>& p, real B,
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real B,
                                                real a[3]) {
     const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
     const real k2 = real(2) * p.kappa * p.i12h;
@@ -78,8 +78,8 @@ struct CM {
   }
 
   // site-form energy density and charge density at an interior site
-  template <typename Tile>
-  __device__ __forceinline__ static void densities(const Tile& T, const StageArgs<real>& p, real B,
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void densities(const Tile& T, const P& p, real B,
                                                    const EdgeW& w, real& e, real& q) {
     const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
     const int ks[4] = {1, -1, 2, -2};
@@ -129,8 +129,8 @@ template <typename real>
 struct AH {
   static constexpr int C = 4;  // 0: Re phi, 1: Im phi, 2: A1, 3: A2
 
-  template <typename Tile>
-  __device__ __forceinline__ static void accel(const Tile& T, const StageArgs<real>& p, real,
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real,
                                                real a[4]) {
     const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
     const real rho = p1 * p1 + p2 * p2, AA = A1 * A1 + A2 * A2;
@@ -161,8 +161,8 @@ struct AH {
     a[0] = -G1; a[1] = -G2; a[2] = -G3; a[3] = -G4;
   }
 
-  template <typename Tile>
-  __device__ __forceinline__ static void densities(const Tile& T, const StageArgs<real>& p, real,
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void densities(const Tile& T, const P& p, real,
                                                    const EdgeW& w, real& e, real& q) {
     const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
     const real rho = p1 * p1 + p2 * p2;
