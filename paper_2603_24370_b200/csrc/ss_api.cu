@@ -96,6 +96,9 @@ void* stage_func(int stage) {
   }
 }
 void* stage_func(int theory, int dtype, int stage) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return stage_func<kCM, double>(stage);
+#endif
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? stage_func<kCM, double>(stage) : stage_func<kCM, float>(stage);
   return dtype == SS_F64 ? stage_func<kAH, double>(stage) : stage_func<kAH, float>(stage);
@@ -114,7 +117,7 @@ struct ss_solver {
   int flags;
   bool fields_set;
   int cur;  // which ping-pong buffer holds (phi, v)
-  int cps;  // chunks per y-segment of the flow kernels
+  int cps[2];  // chunks per y-segment of flow kernels X, Y
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
@@ -132,6 +135,9 @@ namespace {
 
 template <typename real>
 KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return make_stage_node<double>(s, stage, cur);
+#endif
   StageArgs<real> a;
   memset(&a, 0, sizeof(a));
   const double dt = s->dt, h = s->h;
@@ -162,6 +168,10 @@ KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
   a.kappa = real(s->kappa);
   a.K = real(s->K);
   a.lambda = real(s->lambda);
+  a.lap0 = real(60.0 / (12.0 * h * h)); a.lap1 = real(16.0 / (12.0 * h * h));
+  a.lap2 = real(1.0 / (12.0 * h * h));
+  a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
+  a.K2 = real(2.0 * s->K);
   KernelNode n;
   n.func = stage_func(s->theory, s->dtype, stage);
   n.grid = dim3((s->Nx + TX - 1) / TX, (s->Ny + TY - 1) / TY, s->batch);
@@ -223,6 +233,9 @@ void* flow_func_t(int kind) {
   return kind == KX ? (void*)flow_kernel<THEORY, real, KX> : (void*)flow_kernel<THEORY, real, KY>;
 }
 void* flow_func(int theory, int dtype, int kind) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return flow_func_t<kCM, double>(kind);
+#endif
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? flow_func_t<kCM, double>(kind) : flow_func_t<kCM, float>(kind);
   return dtype == SS_F64 ? flow_func_t<kAH, double>(kind) : flow_func_t<kAH, float>(kind);
@@ -232,9 +245,25 @@ int flow_smem_t(int kind) {
   return kind == KX ? FlowCfg<THEORY, real, KX>::SMEM : FlowCfg<THEORY, real, KY>::SMEM;
 }
 int flow_smem(int theory, int dtype, int kind) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return flow_smem_t<kCM, double>(kind);
+#endif
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? flow_smem_t<kCM, double>(kind) : flow_smem_t<kCM, float>(kind);
   return dtype == SS_F64 ? flow_smem_t<kAH, double>(kind) : flow_smem_t<kAH, float>(kind);
+}
+
+template <int THEORY, typename real>
+int flow_threads_t(int kind) {
+  return kind == KX ? FlowCfg<THEORY, real, KX>::THREADS : FlowCfg<THEORY, real, KY>::THREADS;
+}
+int flow_threads(int theory, int dtype, int kind) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return flow_threads_t<kCM, double>(kind);
+#endif
+  if (theory == SS_THEORY_CHIRAL_MAGNET)
+    return dtype == SS_F64 ? flow_threads_t<kCM, double>(kind) : flow_threads_t<kCM, float>(kind);
+  return dtype == SS_F64 ? flow_threads_t<kAH, double>(kind) : flow_threads_t<kAH, float>(kind);
 }
 
 // kernel X (kind KX) evaluates the state in buffer `in`; kernel Y advances `in` -> `in ^ 1`
@@ -255,18 +284,22 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   }
   a.state = s->state();
   a.Bb = (const double*)(s->ws + s->L.off_bb);
-  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg; a.cps = s->cps;
+  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg; a.cps = s->cps[kind];
   a.plane = (long long)s->Nx * s->Ny;
   a.hdt = real(0.5 * dt); a.dt = real(dt);
   a.qdt2 = real(0.25 * (dt * dt)); a.hdt2 = real(0.5 * (dt * dt));
   a.sdt2 = real((dt * dt) / 6.0); a.sdt = real(dt / 6.0);
   a.i12h = real(1.0 / (12.0 * h)); a.i12h2 = real(1.0 / (12.0 * h * h));
   a.kappa = real(s->kappa); a.K = real(s->K); a.lambda = real(s->lambda);
+  a.lap0 = real(60.0 / (12.0 * h * h)); a.lap1 = real(16.0 / (12.0 * h * h));
+  a.lap2 = real(1.0 / (12.0 * h * h));
+  a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
+  a.K2 = real(2.0 * s->K);
   KernelNode n;
   n.func = flow_func(s->theory, s->dtype, kind);
   const int NC = (s->Ny + FR - 1) / FR;
-  n.grid = dim3(s->L.nseg, (NC + s->cps - 1) / s->cps, s->batch);
-  n.block = dim3(FTHREADS, 1, 1);
+  n.grid = dim3(s->L.nseg, (NC + s->cps[kind] - 1) / s->cps[kind], s->batch);
+  n.block = dim3(flow_threads(s->theory, s->dtype, kind), 1, 1);
   n.smem = (size_t)flow_smem(s->theory, s->dtype, kind);
   n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
   n.name = kind == KX ? "flow_x_grad_energy_charge_stage2" : "flow_y_stage34_combine_project_ke";
@@ -274,6 +307,9 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   return true;
 }
 bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
+#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
+  return make_flow_node<double>(s, kind, in, out);
+#endif
   return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out)
                             : make_flow_node<float>(s, kind, in, out);
 }
@@ -418,7 +454,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
     }
   } else {
-    int sms = 148, occ = 1, dev = 0;
+    int sms = 148, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     for (int kind = 0; kind < 2; ++kind) {
@@ -427,14 +463,13 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
       if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
       int o = 1;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, FTHREADS, smem);
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, flow_threads(theory, p->dtype, kind), smem);
       if (!cuda_ok(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor") || o < 1) {
         delete s; return SS_ERR_CUDA;
       }
-      if (kind == KY) occ = o;  // segment the lattice for the heavier kernel
+      s->cps[kind] = p->chunks_per_segment > 0 ? p->chunks_per_segment
+                                               : choose_cps(L.nseg, Ny, s->batch, sms * o);
     }
-    s->cps = p->chunks_per_segment > 0 ? p->chunks_per_segment
-                                       : choose_cps(L.nseg, Ny, s->batch, sms * occ);
   }
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];

@@ -41,6 +41,8 @@ struct StageArgs {
   real dt, sdt2, sdt; // dt, dt^2/6, dt/6
   real i12h, i12h2;   // 1/(12h), 1/(12h^2)
   real kappa, K, lambda;
+  real lap0, lap1, lap2;  // 60, 16, 1 / (12 h^2)
+  real dm1, dm2, K2;      // 2 kappa (8, 1) / (12 h); 2 K
 };
 
 struct ReduceArgs {

@@ -10,13 +10,13 @@
 //       RK4 combine + projections (PAPER.md:123, :129+154), vh = arrested ? 0 : v (eq. 4)
 //
 // A CTA owns a strip of FW = 64 columns and a segment of rows, and marches down the segment in
-// chunks of FR = 4 rows: one thread per site of the chunk.  Per chunk f
+// chunks of FR = 4 rows; a thread owns SPT vertically adjacent sites of the chunk.  Per chunk f
 //   1. TMA (cp.async.bulk.tensor.3d, box {68, 4, C}, zero fill outside the lattice) has put the
 //      raw inputs of chunk f (+2 halo columns each side) into a 2-stage smem buffer;
-//   2. every thread turns its raw site into the two stage fields and writes them into two
-//      16-row smem rings (the x-halo columns are done by 16 extra threads);
+//   2. every thread turns its raw sites into the two stage fields and writes them into two
+//      smem rings of RING rows (the 16 x-halo sites are done by 16 threads);
 //   3. __syncthreads; thread 0 re-arms the stage with the TMA of chunk f+2;
-//   4. every thread evaluates both radius-2 stencils of its site in chunk f-1 from the rings
+//   4. every thread evaluates both radius-2 stencils of its sites in chunk f-1 from the rings
 //      (rows f-1 +- 2 are there), stores the results with coalesced 64-wide row stores and
 //      contributes to the row-segment partial sums of the canonical tree.
 // No y-halo is ever re-read from HBM except one warm-up chunk per segment end.
@@ -30,9 +30,7 @@ namespace ss {
 constexpr int FW = SEG;             // strip width = row segment of the reduction tree
 constexpr int FR = 4;               // rows per chunk
 constexpr int FWP = FW + 2 * HALO;  // ring width
-constexpr int RING = 16;            // ring rows (4 chunks: f-2, f-1, f and the one being filled)
-constexpr int NST = 2;              // TMA stages
-constexpr int FTHREADS = FW * FR;
+constexpr int NST = 2;              // TMA stages of phi, v (a1, a2 of kernel Y: one stage)
 constexpr int KX = 0, KY = 1;
 
 template <typename real>
@@ -50,6 +48,8 @@ struct FlowArgs {
   real sdt2, sdt;                 // dt^2/6, dt/6
   real i12h, i12h2;               // 1/(12h), 1/(12h^2)
   real kappa, K, lambda;
+  real lap0, lap1, lap2;          // 60, 16, 1 / (12 h^2)
+  real dm1, dm2, K2;              // 2 kappa (8, 1) / (12 h); 2 K
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -84,37 +84,81 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
       : "memory");
 }
 
+// tuning switches (defaults = the measured best); X = kernel X, Y = kernel Y
+#ifndef SS_SPT_X
+#define SS_SPT_X 2   // sites per thread
+#endif
+#ifndef SS_SPT_Y
+#define SS_SPT_Y 1
+#endif
+#ifndef SS_RING_X
+#define SS_RING_X 14  // ring rows: >= 14 (chunks f-1, f, f+1 and two rows of f-2 are live)
+#endif
+#ifndef SS_RING_Y
+#define SS_RING_Y 16
+#endif
+#ifndef SS_MINB_X
+#define SS_MINB_X 3   // CTAs per SM the register allocation aims at
+#endif
+#ifndef SS_MINB_Y
+#define SS_MINB_Y 2
+#endif
+
 template <int THEORY, typename real, int KIND>
 struct FlowCfg {
   static constexpr int C = TheoryOf<THEORY, real>::type::C;
-  static constexpr int NARR = KIND == KX ? 2 : 4;
+  static constexpr int SPT = KIND == KX ? SS_SPT_X : SS_SPT_Y;
+  static constexpr int ROWT = FR / SPT;                          // thread rows
+  static constexpr int THREADS = FW * ROWT;
+  static constexpr int RING = KIND == KX ? SS_RING_X : SS_RING_Y;
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
   static constexpr int RAWW = FW + 2 * XPAD;                     // staged width (>= FWP)
   static constexpr int BOXB = C * FR * RAWW * (int)sizeof(real); // bytes one TMA box delivers
   static constexpr int ARRB = (BOXB + 127) / 128 * 128;          // 128-byte aligned slot
+  static constexpr int NARR = KIND == KX ? 2 : 4;                // phi, v (, a1, a2)
   static constexpr int STAGEB = NARR * ARRB;
-  static constexpr int RINGN = C * RING * FWP;                   // elements of one ring
   static constexpr int OFF_RING = NST * STAGEB;
+  static constexpr int RP = RING * FWP;                          // elements of one ring plane
+  static constexpr int RINGN = C * RP;                           // elements of one ring
   static constexpr int OFF_RED = OFF_RING + 2 * RINGN * (int)sizeof(real);
-  static constexpr int OFF_BAR = OFF_RED + 2 * FR * (int)sizeof(double);
+  static constexpr int OFF_BAR = OFF_RED + 2 * 2 * FR * 2 * (int)sizeof(double);
   static constexpr int SMEM = OFF_BAR + NST * 8;
-  static constexpr int MINB = SMEM <= 110 * 1024 ? 2 : 1;        // CTAs per SM (227 KB)
+  static constexpr int WANTB = KIND == KX ? SS_MINB_X : SS_MINB_Y;
+  static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
+  static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTB ? FITB : WANTB);
+  static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small for a single barrier");
+  __device__ __forceinline__ static int ring_row(int gy) {       // gy >= -RING
+    return (RING & (RING - 1)) == 0 ? (gy & (RING - 1)) : (int)((unsigned)(gy + RING) % RING);
+  }
 };
 
+// combined aligned pairwise tree of two quantities over the 32 lanes: even lanes end with the
+// sum of a, odd lanes with the sum of b (5 shuffles instead of 10; IEEE addition commutes)
+__device__ __forceinline__ double warp_tree2(double a, double b, int lane) {
+  const bool odd = lane & 1;
+  const double give = odd ? a : b;
+  double mine = (odd ? b : a) + __shfl_xor_sync(0xffffffffu, give, 1);
+#pragma unroll
+  for (int o = 2; o < 32; o <<= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
+  return mine;
+}
+
 template <int THEORY, typename real, int KIND>
-__global__ void __launch_bounds__(FTHREADS, FlowCfg<THEORY, real, KIND>::MINB)
+__global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
+                                  FlowCfg<THEORY, real, KIND>::MINB)
     flow_kernel(const __grid_constant__ FlowArgs<real> p) {
   using Th = typename TheoryOf<THEORY, real>::type;
   using Cfg = FlowCfg<THEORY, real, KIND>;
-  constexpr int C = Cfg::C;
+  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT;
+  constexpr int NQ = KIND == KX ? 2 : 1;  // partial-sum quantities
   extern __shared__ __align__(128) unsigned char smem[];
   real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3
   real* ringB = ringA + Cfg::RINGN;                             // X: phi2   Y: phi4
-  double* red = reinterpret_cast<double*>(smem + Cfg::OFF_RED); // [2][FR]
+  double* red = reinterpret_cast<double*>(smem + Cfg::OFF_RED); // [2 parity][2 q][FR][2 halves]
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + Cfg::OFF_BAR);
 
   const int tid = threadIdx.x;
-  const int tx = tid & (FW - 1), r = tid >> 6, lane = tid & 31;
+  const int tx = tid & (FW - 1), r0 = (tid >> 6) * SPT, lane = tid & 31;  // rows r0 .. r0+SPT-1
   const int Nx = p.Nx, Ny = p.Ny;
   const int b = blockIdx.z, x0 = blockIdx.x * FW;
   const int NC = (Ny + FR - 1) / FR;
@@ -145,134 +189,175 @@ __global__ void __launch_bounds__(FTHREADS, FlowCfg<THEORY, real, KIND>::MINB)
   if (tid == 0)
     for (int f = f0; f < f0 + NST && f <= f1; ++f) issue(f);
 
-  // raw site -> the two stage fields in the rings; returns the pointwise RK4 data of the site
-  real keep_new[2 * C], keep_old[2 * C];
+  // pointwise RK4 data of the thread's sites, carried from their fill to their stencil (Y):
+  // [0,C) = (phi + dt vh) + dt^2/6 (a1 + a2),  [C,2C) = vh + dt/6 (a1 + 2 a2)
+  real keep_new[SPT][2 * C], keep_old[SPT][2 * C];
 #pragma unroll
-  for (int c = 0; c < 2 * C; ++c) keep_new[c] = keep_old[c] = real(0);
+  for (int k = 0; k < SPT; ++k)
+#pragma unroll
+    for (int c = 0; c < 2 * C; ++c) keep_new[k][c] = keep_old[k][c] = real(0);
 
-  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, bool keep) {
+  // raw site (row, lx) of chunk f -> the two stage fields in the rings
+  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, real* keep) {
+    constexpr int RW = Cfg::RAWW;
     const int gx = x0 - HALO + lx, gy = f * FR + row;
     const bool inter = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
-    constexpr int RW = Cfg::RAWW;
     const int ro = row * RW + lx + (Cfg::XPAD - HALO);
     const real* rphi = reinterpret_cast<const real*>(st);
     const real* rvel = reinterpret_cast<const real*>(st + Cfg::ARRB);
-    real ph[C], A[C], Bf[C];
+    real A[C], Bf[C];
 #pragma unroll
-    for (int c = 0; c < C; ++c) ph[c] = rphi[c * FR * RW + ro];
-    if (KIND == KX) {
+    for (int c = 0; c < C; ++c) A[c] = Bf[c] = rphi[c * FR * RW + ro];
+    if (inter) {  // halo sites of every stage field are the frozen halo
+      if (KIND == KX) {
 #pragma unroll
-      for (int c = 0; c < C; ++c) {
-        A[c] = ph[c];
-        Bf[c] = ph[c] + p.hdt * rvel[c * FR * RW + ro];
-      }
-      Th::project_field(Bf);
-    } else {
-      const real* ra1 = reinterpret_cast<const real*>(st + 2 * Cfg::ARRB);
-      const real* ra2 = reinterpret_cast<const real*>(st + 3 * Cfg::ARRB);
-      real k0[C], k1[C];
+        for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * rvel[c * FR * RW + ro];
+        Th::project_field(Bf);
+      } else {
+        const real* ra1 = reinterpret_cast<const real*>(st + 2 * Cfg::ARRB);
+        const real* ra2 = reinterpret_cast<const real*>(st + 3 * Cfg::ARRB);
 #pragma unroll
-      for (int c = 0; c < C; ++c) {
-        const real a1 = ra1[c * FR * RW + ro];
-        const real vh = vz ? real(0) : rvel[c * FR * RW + ro];
-        const real a2 = vz ? a1 : ra2[c * FR * RW + ro];
-        A[c] = (ph[c] + p.hdt * vh) + p.qdt2 * a1;
-        const real base = ph[c] + p.dt * vh;
-        Bf[c] = base + p.hdt2 * a2;
-        k0[c] = base + p.sdt2 * (a1 + a2);
-        k1[c] = vh + p.sdt * (a1 + real(2) * a2);
-      }
-      Th::project_field(A);
-      Th::project_field(Bf);
-      if (keep) {
-#pragma unroll
-        for (int c = 0; c < C; ++c) { keep_new[c] = k0[c]; keep_new[C + c] = k1[c]; }
+        for (int c = 0; c < C; ++c) {
+          const real ph = A[c];
+          const real a1 = ra1[c * FR * RW + ro];
+          const real vh = vz ? real(0) : rvel[c * FR * RW + ro];
+          const real a2 = vz ? a1 : ra2[c * FR * RW + ro];
+          A[c] = (ph + p.hdt * vh) + p.qdt2 * a1;
+          const real base = ph + p.dt * vh;
+          Bf[c] = base + p.hdt2 * a2;
+          if (keep) {
+            keep[c] = base + p.sdt2 * (a1 + a2);
+            keep[C + c] = vh + p.sdt * (a1 + real(2) * a2);
+          }
+        }
+        Th::project_field(A);
+        Th::project_field(Bf);
       }
     }
-    const int wo = (gy & (RING - 1)) * FWP + lx;
+    const int wo = Cfg::ring_row(gy) * FWP + lx;
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      ringA[c * RING * FWP + wo] = inter ? A[c] : ph[c];
-      ringB[c * RING * FWP + wo] = inter ? Bf[c] : ph[c];
+      ringA[c * RP + wo] = A[c];
+      ringB[c * RP + wo] = Bf[c];
     }
   };
+
+  // row-segment partial sums of chunk sc (written by the two warps of each row into `red`)
+  auto flush_partials = [&](int sc, int par) {
+    if (tid < NQ * FR) {
+      const int q = tid / FR, row = tid % FR, gy = sc * FR + row;
+      if (gy < Ny) {
+        const double* rr = red + ((par * 2 + q) * FR + row) * 2;
+        double* dst = q == 0 ? p.part0 : p.part1;
+        dst[((long long)b * Ny + gy) * p.nseg + blockIdx.x] = rr[0] + rr[1];
+      }
+    }
+  };
+
+  const int gx = x0 + tx;
+  const bool xin = gx >= HALO && gx < Nx - HALO;
+  const bool xedge = gx < 2 * HALO || gx >= Nx - 2 * HALO;
 
   for (int f = f0; f <= ce; ++f) {
     if (f <= f1) {
       const int k = f - f0;
       const unsigned char* st = smem + (k % NST) * Cfg::STAGEB;
       mbar_wait(&full[k % NST], (uint32_t)((k / NST) & 1));
-      fill_site(st, f, r, tx + HALO, true);
+#pragma unroll
+      for (int k2 = 0; k2 < SPT; ++k2) fill_site(st, f, r0 + k2, tx + HALO, keep_new[k2]);
       if (tid < 4 * FR) {
         const int q = tid & 3;
-        fill_site(st, f, tid >> 2, q < 2 ? q : FW + q, false);
+        fill_site(st, f, tid >> 2, q < 2 ? q : FW + q, nullptr);
       }
     }
     __syncthreads();
     if (tid == 0 && f + NST <= f1) issue(f + NST);
 
     const int sc = f - 1;
+    if (sc - 1 >= cs && sc - 1 < ce) flush_partials(sc - 1, (f - 1) & 1);
     if (sc >= cs && sc < ce) {
-      const int gx = x0 + tx, gy = sc * FR + r;
-      const bool active = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
-      double s0 = 0.0, s1 = 0.0;
-      if (active) {
-        int ro[5];
+      const int gy0 = sc * FR + r0;
+      // ring offsets of rows gy0-2 .. gy0+SPT+1 at the thread's column
+      int rw[SPT + 4];
 #pragma unroll
-        for (int d = 0; d < 5; ++d) ro[d] = ((gy + d - 2) & (RING - 1)) * FWP + tx + HALO;
-        auto TA = [&](int c, int dy, int dx) -> real { return ringA[c * RING * FWP + ro[dy + 2] + dx]; };
-        auto TB = [&](int c, int dy, int dx) -> real { return ringB[c * RING * FWP + ro[dy + 2] + dx]; };
-        const long long o = (long long)b * C * p.plane + (long long)gy * Nx + gx;
-        real aA[C], aB[C];
-        Th::accel(TA, p, Bz, aA);
-        if (KIND == KX) {
+      for (int j = 0; j < SPT + 4; ++j) rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
+      double s0[SPT], s1[SPT];
 #pragma unroll
-          for (int c = 0; c < C; ++c) p.out0[o + c * p.plane] = aA[c];
-          real e, q;
-          EdgeW w(gx, gy, Nx, Ny);
-          Th::densities(TA, p, Bz, w, e, q);
-          s0 = double(e);
-          s1 = double(q);
-          Th::accel(TB, p, Bz, aB);
+      for (int k = 0; k < SPT; ++k) {
+        const int gy = gy0 + k;
+        s0[k] = s1[k] = 0.0;
+        if (xin && gy >= HALO && gy < Ny - HALO) {
+          auto TA = [&](int c, int dy, int dx) -> real { return ringA[c * RP + rw[k + dy + 2] + dx]; };
+          auto TB = [&](int c, int dy, int dx) -> real { return ringB[c * RP + rw[k + dy + 2] + dx]; };
+          const long long o = (long long)b * C * p.plane + (long long)gy * Nx + gx;
+          real* o0 = p.out0 + o;
+          real* o1 = p.out1 + o;
+          real aA[C], aB[C];
+          Th::accel(TA, p, Bz, aA);
+          if (KIND == KX) {
+            real e, q;
+#ifdef SS_EXP_NODENS
+            e = aA[0]; q = aA[1];
+#else
+            if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO)
+              Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
+            else
+              Th::densities(TA, p, Bz, BulkW(), e, q);
+#endif
 #pragma unroll
-          for (int c = 0; c < C; ++c) p.out1[o + c * p.plane] = aB[c];
-        } else {
-          Th::accel(TB, p, Bz, aB);
-          real fn[C], u[C];
+            for (int c = 0; c < C; ++c) o0[c * p.plane] = aA[c];
+            s0[k] = double(e);
+            s1[k] = double(q);
+#ifdef SS_EXP_NOB
 #pragma unroll
-          for (int c = 0; c < C; ++c) {
-            fn[c] = keep_old[c] + p.sdt2 * aA[c];
-            u[c] = keep_old[C + c] + p.sdt * (real(2) * aA[c] + aB[c]);
+            for (int c = 0; c < C; ++c) aB[c] = TB(c, 0, 0) + aA[c];
+#else
+            Th::accel(TB, p, Bz, aB);
+#endif
+#pragma unroll
+            for (int c = 0; c < C; ++c) o1[c * p.plane] = aB[c];
+          } else {
+            Th::accel(TB, p, Bz, aB);
+            real fn[C], u[C];
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+              fn[c] = keep_old[k][c] + p.sdt2 * aA[c];
+              u[c] = keep_old[k][C + c] + p.sdt * (real(2) * aA[c] + aB[c]);
+            }
+            Th::project_field(fn);
+            Th::project_velocity(u, fn);
+            real v2 = real(0);
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+              o0[c * p.plane] = fn[c];
+              o1[c * p.plane] = u[c];
+              v2 += u[c] * u[c];
+            }
+            s0[k] = 0.5 * double(v2);
           }
-          Th::project_field(fn);
-          Th::project_velocity(u, fn);
-          real v2 = real(0);
-#pragma unroll
-          for (int c = 0; c < C; ++c) {
-            p.out0[o + c * p.plane] = fn[c];
-            p.out1[o + c * p.plane] = u[c];
-            v2 += u[c] * u[c];
-          }
-          s0 = 0.5 * double(v2);
         }
       }
-      // row-segment partial sums: aligned pairwise tree over the 64 sites of (row, strip)
-      s0 = warp_tree(s0);
-      if (KIND == KX) s1 = warp_tree(s1);
-      if (lane == 0 && tx >= 32) {
-        red[r] = s0;
-        if (KIND == KX) red[FR + r] = s1;
-      }
-      asm volatile("bar.sync %0, 64;" ::"r"(1 + r) : "memory");
-      if (tx == 0 && gy < Ny) {
-        const long long po = ((long long)b * Ny + gy) * p.nseg + blockIdx.x;
-        p.part0[po] = s0 + red[r];
-        if (KIND == KX) p.part1[po] = s1 + red[FR + r];
+      // aligned pairwise tree over the 32 sites of the warp; the two halves of the 64-site row
+      // segment are added (low + high) by flush_partials after the next barrier
+#pragma unroll
+      for (int k = 0; k < SPT; ++k) {
+        double* rr = red + (((f & 1) * 2) * FR + r0 + k) * 2 + (tx >> 5);
+        if (KIND == KX) {
+          const double t = warp_tree2(s0[k], s1[k], lane);
+          if (lane < 2) rr[lane * FR * 2] = t;
+        } else {
+          const double t = warp_tree(s0[k]);
+          if (lane == 0) rr[0] = t;
+        }
       }
     }
 #pragma unroll
-    for (int c = 0; c < 2 * C; ++c) keep_old[c] = keep_new[c];
+    for (int k = 0; k < SPT; ++k)
+#pragma unroll
+      for (int c = 0; c < 2 * C; ++c) keep_old[k][c] = keep_new[k][c];
   }
+  __syncthreads();
+  if (ce - 1 >= cs) flush_partials(ce - 1, ce & 1);
 }
 
 }  // namespace ss

@@ -20,6 +20,14 @@ struct EdgeW {
     y[2] = (gy + 2 < Ny - HALO) ? 1 : 2;
     y[3] = (gy - 2 >= HALO) ? 1 : 2;
   }
+  __device__ __forceinline__ int wx(int s) const { return x[s]; }
+  __device__ __forceinline__ int wy(int s) const { return y[s]; }
+};
+
+// all neighbours interior (sites at least 4 from every edge): the weights fold away
+struct BulkW {
+  __device__ __forceinline__ constexpr int wx(int) const { return 1; }
+  __device__ __forceinline__ constexpr int wy(int) const { return 1; }
 };
 
 // eq. (1) numerators: 12h * D f = 8 (f+1 - f-1) - (f+2 - f-2)
@@ -62,25 +70,33 @@ struct CM {
   static constexpr int C = 3;
 
   // a = -(G - (G.n) n),  G = -(Lx+Ly) n + 2 kappa (Dy n3, -Dx n3, Dx n2 - Dy n1) - (B + 2K n3) e3
+  // with the stencil weights folded into five constants (kernel parameters, so they are
+  // constant-bank operands): lap0/1/2 = 60, 16, 1 /(12h^2); dm1/2 = 2 kappa (8, 1)/(12h).
   template <typename Tile, typename P>
-  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real B,
-                                               real a[3]) {
+  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real B, real a[3]) {
     const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
-    const real k2 = real(2) * p.kappa * p.i12h;
-    real G1 = -(Lxn<real>(T, 0) + Lyn<real>(T, 0)) * p.i12h2 + k2 * Dyn<real>(T, 2);
-    real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 - k2 * Dxn<real>(T, 2);
-    real G3 = -(Lxn<real>(T, 2) + Lyn<real>(T, 2)) * p.i12h2 +
-              k2 * (Dxn<real>(T, 1) - Dyn<real>(T, 0)) - (B + real(2) * p.K * n3);
-    const real gn = (G1 * n1 + G2 * n2) + G3 * n3;
-    a[0] = gn * n1 - G1;
-    a[1] = gn * n2 - G2;
-    a[2] = gn * n3 - G3;
+    real G[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {  // -(Lx + Ly) n_c
+      const real s1 = (T(c, 0, 1) + T(c, 0, -1)) + (T(c, 1, 0) + T(c, -1, 0));
+      const real s2 = (T(c, 0, 2) + T(c, 0, -2)) + (T(c, 2, 0) + T(c, -2, 0));
+      G[c] = p.lap2 * s2 + (p.lap0 * T(c, 0, 0) - p.lap1 * s1);
+    }
+    G[0] += p.dm1 * (T(2, 1, 0) - T(2, -1, 0)) - p.dm2 * (T(2, 2, 0) - T(2, -2, 0));
+    G[1] -= p.dm1 * (T(2, 0, 1) - T(2, 0, -1)) - p.dm2 * (T(2, 0, 2) - T(2, 0, -2));
+    G[2] += p.dm1 * ((T(1, 0, 1) - T(1, 0, -1)) - (T(0, 1, 0) - T(0, -1, 0))) -
+            p.dm2 * ((T(1, 0, 2) - T(1, 0, -2)) - (T(0, 2, 0) - T(0, -2, 0)));
+    G[2] -= B + p.K2 * n3;
+    const real gn = (G[0] * n1 + G[1] * n2) + G[2] * n3;
+    a[0] = gn * n1 - G[0];
+    a[1] = gn * n2 - G[1];
+    a[2] = gn * n3 - G[2];
   }
 
   // site-form energy density and charge density at an interior site
-  template <typename Tile, typename P>
+  template <typename Tile, typename P, typename W>
   __device__ __forceinline__ static void densities(const Tile& T, const P& p, real B,
-                                                   const EdgeW& w, real& e, real& q) {
+                                                   const W& w, real& e, real& q) {
     const real n1 = T(0, 0, 0), n2 = T(1, 0, 0), n3 = T(2, 0, 0);
     const int ks[4] = {1, -1, 2, -2};
     const real J4[4] = {real(4) * p.i12h2, real(4) * p.i12h2, real(-0.25) * p.i12h2,
@@ -94,14 +110,14 @@ struct CM {
         const real d1 = n1 - m1, d2 = n2 - m2, d3 = n3 - m3;
         const real ex = J4[s] * (d1 * d1 + d2 * d2 + d3 * d3);
         const real cr = n3 * m2 - n2 * m3;  // n_i . (e_x x n_j)
-        acc += real(w.x[s]) * (ex + p.kappa * ck[s] * cr);
+        acc += real(w.wx(s)) * (ex + p.kappa * ck[s] * cr);
       }
       {  // y neighbour
         const real m1 = T(0, ks[s], 0), m2 = T(1, ks[s], 0), m3 = T(2, ks[s], 0);
         const real d1 = n1 - m1, d2 = n2 - m2, d3 = n3 - m3;
         const real ex = J4[s] * (d1 * d1 + d2 * d2 + d3 * d3);
         const real cr = n1 * m3 - n3 * m1;  // n_i . (e_y x n_j)
-        acc += real(w.y[s]) * (ex + p.kappa * ck[s] * cr);
+        acc += real(w.wy(s)) * (ex + p.kappa * ck[s] * cr);
       }
     }
     e = acc + B * (real(1) - n3) + p.K * (real(1) - n3 * n3);
@@ -161,9 +177,9 @@ struct AH {
     a[0] = -G1; a[1] = -G2; a[2] = -G3; a[3] = -G4;
   }
 
-  template <typename Tile, typename P>
+  template <typename Tile, typename P, typename W>
   __device__ __forceinline__ static void densities(const Tile& T, const P& p, real,
-                                                   const EdgeW& w, real& e, real& q) {
+                                                   const W& w, real& e, real& q) {
     const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
     const real rho = p1 * p1 + p2 * p2;
     const int ks[4] = {1, -1, 2, -2};
@@ -178,14 +194,14 @@ struct AH {
         const real q1 = T(0, 0, ks[s]), q2 = T(1, 0, ks[s]);
         const real d1 = p1 - q1, d2 = p2 - q2, dA = A2 - T(3, 0, ks[s]);
         const real im = p1 * q2 - p2 * q1;
-        acc += real(w.x[s]) * (J4[s] * (d1 * d1 + d2 * d2) -
+        acc += real(w.wx(s)) * (J4[s] * (d1 * d1 + d2 * d2) -
                                real(0.5) * ck[s] * (A1 + T(2, 0, ks[s])) * im + J4[s] * (dA * dA));
       }
       {  // y bond: A_mu = A2, transverse A1
         const real q1 = T(0, ks[s], 0), q2 = T(1, ks[s], 0);
         const real d1 = p1 - q1, d2 = p2 - q2, dA = A1 - T(2, ks[s], 0);
         const real im = p1 * q2 - p2 * q1;
-        acc += real(w.y[s]) * (J4[s] * (d1 * d1 + d2 * d2) -
+        acc += real(w.wy(s)) * (J4[s] * (d1 * d1 + d2 * d2) -
                                real(0.5) * ck[s] * (A2 + T(3, ks[s], 0)) * im + J4[s] * (dA * dA));
       }
     }
@@ -195,7 +211,7 @@ struct AH {
     for (int sk = 0; sk < 4; ++sk)
 #pragma unroll
       for (int sl = 0; sl < 4; ++sl) {
-        const real wt = (w.x[sk] == 1 && w.y[sl] == 1) ? real(1) : real(2);
+        const real wt = (w.wx(sk) == 1 && w.wy(sl) == 1) ? real(1) : real(2);
         const real cc = ck[sk] * ck[sl] * wt;
         W1 += cc * T(2, ks[sl], ks[sk]);
         W2 += cc * T(3, ks[sl], ks[sk]);
