@@ -229,6 +229,21 @@ KERNEL_UNITS = {
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
 
+def max_over_ranks(values, dist=None, device="cpu"):
+    """Element-wise MAX over all ranks of a list of floats (identity without a process group)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def job_value(world, sites_per_rank, steps, ms):
+    """Whole-job site-updates/s of `world` replicas that each did `steps` steps in `ms` (max)."""
+    return world * sites_per_rank * steps / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -275,11 +290,8 @@ def run_ours(args):
     clocks = sampler.stop()
     launches = s.launch_count() - n0
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * sites * args.steps / (ms * 1e-3)
+    ms = max_over_ranks([ms], dist if world > 1 else None, dev)[0]
+    value = job_value(world, sites, args.steps, ms)
     st = s.status()
 
     # ---- per-kernel CUDA-event times of the same step (kernels launched one by one)
@@ -343,10 +355,7 @@ def run_e2e(r, args):
     job(min(K, 3))                                        # warm the pinned paths
     t, E, Q = job(K)
     trt = min(job(1)[0] for _ in range(3))
-    if r["world"] > 1:
-        tt = torch.tensor([t, trt], device=dev, dtype=torch.float64)
-        r["dist"].all_reduce(tt, op=r["dist"].ReduceOp.MAX)
-        t, trt = float(tt[0]), float(tt[1])
+    t, trt = max_over_ranks([t, trt], r["dist"] if r["world"] > 1 else None, dev)
     nsc = 2 * 8 * r["w"].batch
     return {
         "value": r["world"] * r["sites"] * K / t, "unit": UNIT,
