@@ -295,6 +295,9 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   a.lap2 = real(1.0 / (12.0 * h * h));
   a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
   a.K2 = real(2.0 * s->K);
+  a.jA = real((16.0 / 12.0) / (4.0 * h * h)); a.jB = real((-1.0 / 12.0) / (4.0 * h * h));
+  a.hk = real(s->kappa / (12.0 * h));
+  a.qs = real(1.0 / (4.0 * 3.14159265358979323846 * (12.0 * h) * (12.0 * h)));
   KernelNode n;
   n.func = flow_func(s->theory, s->dtype, kind);
   const int NC = (s->Ny + FR - 1) / FR;

@@ -30,7 +30,6 @@ namespace ss {
 constexpr int FW = SEG;             // strip width = row segment of the reduction tree
 constexpr int FR = 4;               // rows per chunk
 constexpr int FWP = FW + 2 * HALO;  // ring width
-constexpr int NST = 2;              // TMA stages of phi, v (a1, a2 of kernel Y: one stage)
 constexpr int KX = 0, KY = 1;
 
 template <typename real>
@@ -50,6 +49,7 @@ struct FlowArgs {
   real kappa, K, lambda;
   real lap0, lap1, lap2;          // 60, 16, 1 / (12 h^2)
   real dm1, dm2, K2;              // 2 kappa (8, 1) / (12 h); 2 K
+  real jA, jB, hk, qs;            // J1/4h^2, J2/4h^2, kappa/(12h), 1/(4 pi (12h)^2)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -89,19 +89,25 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 #define SS_SPT_X 2   // sites per thread
 #endif
 #ifndef SS_SPT_Y
-#define SS_SPT_Y 1
+#define SS_SPT_Y 2
 #endif
 #ifndef SS_RING_X
 #define SS_RING_X 14  // ring rows: >= 14 (chunks f-1, f, f+1 and two rows of f-2 are live)
 #endif
 #ifndef SS_RING_Y
-#define SS_RING_Y 16
+#define SS_RING_Y 14
+#endif
+#ifndef SS_NST_X
+#define SS_NST_X 2    // TMA stages (chunks in flight while one is worked on)
+#endif
+#ifndef SS_NST_Y
+#define SS_NST_Y 1    // one stage + 3 CTAs/SM beats two stages + 2 CTAs/SM for kernel Y
 #endif
 #ifndef SS_MINB_X
 #define SS_MINB_X 3   // CTAs per SM the register allocation aims at
 #endif
 #ifndef SS_MINB_Y
-#define SS_MINB_Y 2
+#define SS_MINB_Y 3
 #endif
 
 template <int THEORY, typename real, int KIND>
@@ -111,6 +117,7 @@ struct FlowCfg {
   static constexpr int ROWT = FR / SPT;                          // thread rows
   static constexpr int THREADS = FW * ROWT;
   static constexpr int RING = KIND == KX ? SS_RING_X : SS_RING_Y;
+  static constexpr int NST = KIND == KX ? SS_NST_X : SS_NST_Y;
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
   static constexpr int RAWW = FW + 2 * XPAD;                     // staged width (>= FWP)
   static constexpr int BOXB = C * FR * RAWW * (int)sizeof(real); // bytes one TMA box delivers
@@ -149,7 +156,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     flow_kernel(const __grid_constant__ FlowArgs<real> p) {
   using Th = typename TheoryOf<THEORY, real>::type;
   using Cfg = FlowCfg<THEORY, real, KIND>;
-  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT;
+  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT, NST = Cfg::NST;
   constexpr int NQ = KIND == KX ? 2 : 1;  // partial-sum quantities
   extern __shared__ __align__(128) unsigned char smem[];
   real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3
@@ -293,30 +300,23 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
           real* o0 = p.out0 + o;
           real* o1 = p.out1 + o;
           real aA[C], aB[C];
-          Th::accel(TA, p, Bz, aA);
           if (KIND == KX) {
             real e, q;
-#ifdef SS_EXP_NODENS
-            e = aA[0]; q = aA[1];
-#else
-            if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO)
+            if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
+              Th::accel(TA, p, Bz, aA);
               Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
-            else
-              Th::densities(TA, p, Bz, BulkW(), e, q);
-#endif
+            } else {
+              Th::accel_densities_bulk(TA, p, Bz, aA, e, q);
+            }
 #pragma unroll
             for (int c = 0; c < C; ++c) o0[c * p.plane] = aA[c];
             s0[k] = double(e);
             s1[k] = double(q);
-#ifdef SS_EXP_NOB
-#pragma unroll
-            for (int c = 0; c < C; ++c) aB[c] = TB(c, 0, 0) + aA[c];
-#else
             Th::accel(TB, p, Bz, aB);
-#endif
 #pragma unroll
             for (int c = 0; c < C; ++c) o1[c * p.plane] = aB[c];
           } else {
+            Th::accel(TA, p, Bz, aA);
             Th::accel(TB, p, Bz, aB);
             real fn[C], u[C];
 #pragma unroll

@@ -93,6 +93,50 @@ struct CM {
     a[2] = gn * n3 - G[2];
   }
 
+  // accel + site-form energy density + charge density of a site whose neighbours are all
+  // interior (weights 1): the eq. (1) numerators d_x n, d_y n are formed once and serve the DMI
+  // force, the DMI energy kappa n.(curl_h n) and the charge; the exchange energy keeps the
+  // plain |n_i - n_j|^2 form (valid for non-unit fields), summed per neighbour shell.
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real B,
+                                                              real a[3], real& e, real& q) {
+    const real n[3] = {T(0, 0, 0), T(1, 0, 0), T(2, 0, 0)};
+    real G[3], dx[3], dy[3];
+    real sA0 = real(0), sA1 = real(0), sB0 = real(0), sB1 = real(0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const real xp1 = T(c, 0, 1), xm1 = T(c, 0, -1), yp1 = T(c, 1, 0), ym1 = T(c, -1, 0);
+      const real xp2 = T(c, 0, 2), xm2 = T(c, 0, -2), yp2 = T(c, 2, 0), ym2 = T(c, -2, 0);
+      const real s1 = (xp1 + xm1) + (yp1 + ym1);
+      const real s2 = (xp2 + xm2) + (yp2 + ym2);
+      G[c] = p.lap2 * s2 + (p.lap0 * n[c] - p.lap1 * s1);
+      dx[c] = real(8) * (xp1 - xm1) - (xp2 - xm2);
+      dy[c] = real(8) * (yp1 - ym1) - (yp2 - ym2);
+      real d;
+      d = n[c] - xp1; sA0 += d * d;
+      d = n[c] - xm1; sA1 += d * d;
+      d = n[c] - yp1; sA0 += d * d;
+      d = n[c] - ym1; sA1 += d * d;
+      d = n[c] - xp2; sB0 += d * d;
+      d = n[c] - xm2; sB1 += d * d;
+      d = n[c] - yp2; sB0 += d * d;
+      d = n[c] - ym2; sB1 += d * d;
+    }
+    G[0] += p.dm2 * dy[2];
+    G[1] -= p.dm2 * dx[2];
+    G[2] += p.dm2 * (dx[1] - dy[0]) - (B + p.K2 * n[2]);
+    const real gn = (G[0] * n[0] + G[1] * n[1]) + G[2] * n[2];
+    a[0] = gn * n[0] - G[0];
+    a[1] = gn * n[1] - G[1];
+    a[2] = gn * n[2] - G[2];
+    const real curl = (n[2] * dx[1] - n[1] * dx[2]) + (n[0] * dy[2] - n[2] * dy[0]);
+    e = (p.jA * (sA0 + sA1) + p.jB * (sB0 + sB1)) + p.hk * curl +
+        (B * (real(1) - n[2]) + p.K * (real(1) - n[2] * n[2]));
+    const real c1 = dx[1] * dy[2] - dx[2] * dy[1], c2 = dx[2] * dy[0] - dx[0] * dy[2],
+               c3 = dx[0] * dy[1] - dx[1] * dy[0];
+    q = p.qs * ((n[0] * c1 + n[1] * c2) + n[2] * c3);
+  }
+
   // site-form energy density and charge density at an interior site
   template <typename Tile, typename P, typename W>
   __device__ __forceinline__ static void densities(const Tile& T, const P& p, real B,
@@ -218,6 +262,13 @@ struct AH {
       }
     e = acc + real(0.5) * (A2 * W1 + A1 * W2);
     q = real(0.15915494309189535) * p.i12h * (Dxn<real>(T, 3) - Dyn<real>(T, 2));
+  }
+
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real B,
+                                                              real a[4], real& e, real& q) {
+    accel(T, p, B, a);
+    densities(T, p, B, BulkW(), e, q);
   }
 
   __device__ __forceinline__ static void project_field(real*) {}
