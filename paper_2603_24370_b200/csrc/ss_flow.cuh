@@ -289,48 +289,78 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 #pragma unroll
       for (int j = 0; j < SPT + 4; ++j) rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
       double s0[SPT], s1[SPT];
+      bool act[SPT];
+      real aA[SPT][C];
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
-        const int gy = gy0 + k;
         s0[k] = s1[k] = 0.0;
-        if (xin && gy >= HALO && gy < Ny - HALO) {
-          auto TA = [&](int c, int dy, int dx) -> real { return ringA[c * RP + rw[k + dy + 2] + dx]; };
-          auto TB = [&](int c, int dy, int dx) -> real { return ringB[c * RP + rw[k + dy + 2] + dx]; };
-          const long long o = (long long)b * C * p.plane + (long long)gy * Nx + gx;
-          real* o0 = p.out0 + o;
-          real* o1 = p.out1 + o;
-          real aA[C], aB[C];
+        act[k] = xin && gy0 + k >= HALO && gy0 + k < Ny - HALO;
+      }
+      const long long o = (long long)b * C * p.plane + (long long)gy0 * Nx + gx;
+      real* o0 = p.out0 + o;
+      real* o1 = p.out1 + o;
+      // The SPT sites of a thread share their column: its SPT+4 ring values per component are
+      // loaded once into registers; only the x-neighbours are read per site.
+      real col[C][SPT + 4];
+      // ---- ring A (X: phi -> a1, e, q    Y: phi3 -> a3)
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringA[c * RP + rw[j]];
+#pragma unroll
+      for (int k = 0; k < SPT; ++k) {
+        if (act[k]) {
+          const int gy = gy0 + k;
+          auto TA = [&](int c, int dy, int dx) -> real {
+            return dx == 0 ? col[c][k + dy + 2] : ringA[c * RP + rw[k + dy + 2] + dx];
+          };
           if (KIND == KX) {
             real e, q;
             if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
-              Th::accel(TA, p, Bz, aA);
+              Th::accel(TA, p, Bz, aA[k]);
               Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
             } else {
-              Th::accel_densities_bulk(TA, p, Bz, aA, e, q);
+              Th::accel_densities_bulk(TA, p, Bz, aA[k], e, q);
             }
 #pragma unroll
-            for (int c = 0; c < C; ++c) o0[c * p.plane] = aA[c];
+            for (int c = 0; c < C; ++c) o0[c * p.plane + k * Nx] = aA[k][c];
             s0[k] = double(e);
             s1[k] = double(q);
-            Th::accel(TB, p, Bz, aB);
-#pragma unroll
-            for (int c = 0; c < C; ++c) o1[c * p.plane] = aB[c];
           } else {
-            Th::accel(TA, p, Bz, aA);
-            Th::accel(TB, p, Bz, aB);
+            Th::accel(TA, p, Bz, aA[k]);
+          }
+        }
+      }
+      // ---- ring B (X: phi2 -> a2    Y: phi4 -> a4, RK4 combine, projections, KE)
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringB[c * RP + rw[j]];
+#pragma unroll
+      for (int k = 0; k < SPT; ++k) {
+        if (act[k]) {
+          auto TB = [&](int c, int dy, int dx) -> real {
+            return dx == 0 ? col[c][k + dy + 2] : ringB[c * RP + rw[k + dy + 2] + dx];
+          };
+          real aB[C];
+          Th::accel(TB, p, Bz, aB);
+          if (KIND == KX) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) o1[c * p.plane + k * Nx] = aB[c];
+          } else {
             real fn[C], u[C];
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-              fn[c] = keep_old[k][c] + p.sdt2 * aA[c];
-              u[c] = keep_old[k][C + c] + p.sdt * (real(2) * aA[c] + aB[c]);
+              fn[c] = keep_old[k][c] + p.sdt2 * aA[k][c];
+              u[c] = keep_old[k][C + c] + p.sdt * (real(2) * aA[k][c] + aB[c]);
             }
             Th::project_field(fn);
             Th::project_velocity(u, fn);
             real v2 = real(0);
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-              o0[c * p.plane] = fn[c];
-              o1[c * p.plane] = u[c];
+              o0[c * p.plane + k * Nx] = fn[c];
+              o1[c * p.plane + k * Nx] = u[c];
               v2 += u[c] * u[c];
             }
             s0[k] = 0.5 * double(v2);
