@@ -264,11 +264,56 @@ struct AH {
     q = real(0.15915494309189535) * p.i12h * (Dxn<real>(T, 3) - Dyn<real>(T, 2));
   }
 
+  // accel + site-form energy density + flux density of a site whose neighbours are all interior:
+  // the bond term -1/2 c_k (A_i + A_j) Im(phi_i* phi_j) is p1 S_2 - p2 S_1 with the sums
+  // S_mu,c = sum_k c_k (A_mu,i + A_mu,j) phi_c,j of the force, and the mixed term is
+  // 1/2 (A2 DxDy A1 + A1 DxDy A2) with the corner sums of the force.
   template <typename Tile, typename P>
-  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real B,
+  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real,
                                                               real a[4], real& e, real& q) {
-    accel(T, p, B, a);
-    densities(T, p, B, BulkW(), e, q);
+    const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
+    const real rho = p1 * p1 + p2 * p2, AA = A1 * A1 + A2 * A2;
+    real Sx1, Sx2, Sy1, Sy2;
+    {
+      const real am2 = T(2, 0, -2) + A1, am1 = T(2, 0, -1) + A1, ap1 = T(2, 0, 1) + A1,
+                 ap2 = T(2, 0, 2) + A1;
+      Sx1 = d1n<real>(am2 * T(0, 0, -2), am1 * T(0, 0, -1), ap1 * T(0, 0, 1), ap2 * T(0, 0, 2));
+      Sx2 = d1n<real>(am2 * T(1, 0, -2), am1 * T(1, 0, -1), ap1 * T(1, 0, 1), ap2 * T(1, 0, 2));
+    }
+    {
+      const real am2 = T(3, -2, 0) + A2, am1 = T(3, -1, 0) + A2, ap1 = T(3, 1, 0) + A2,
+                 ap2 = T(3, 2, 0) + A2;
+      Sy1 = d1n<real>(am2 * T(0, -2, 0), am1 * T(0, -1, 0), ap1 * T(0, 1, 0), ap2 * T(0, 2, 0));
+      Sy2 = d1n<real>(am2 * T(1, -2, 0), am1 * T(1, -1, 0), ap1 * T(1, 1, 0), ap2 * T(1, 2, 0));
+    }
+    const real pot = real(0.5) * p.lambda * (real(1) - rho);
+    const real G1 = -(Lxn<real>(T, 0) + Lyn<real>(T, 0)) * p.i12h2 - (Sx2 + Sy2) * p.i12h +
+                    (AA - pot) * p1;
+    const real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 + (Sx1 + Sy1) * p.i12h +
+                    (AA - pot) * p2;
+    const real ii = p.i12h * p.i12h;
+    const real xyA1 = Dxyn<real>(T, 2), xyA2 = Dxyn<real>(T, 3);
+    const real dxA2 = Dxn<real>(T, 3), dyA1 = Dyn<real>(T, 2);
+    const real G3 = -Lyn<real>(T, 2) * p.i12h2 + xyA2 * ii +
+                    (p2 * Dxn<real>(T, 0) - p1 * Dxn<real>(T, 1)) * p.i12h + A1 * rho;
+    const real G4 = -Lxn<real>(T, 3) * p.i12h2 + xyA1 * ii +
+                    (p2 * Dyn<real>(T, 0) - p1 * Dyn<real>(T, 1)) * p.i12h + A2 * rho;
+    a[0] = -G1; a[1] = -G2; a[2] = -G3; a[3] = -G4;
+    // bond sums per neighbour shell: |phi_i - phi_j|^2 + (transverse A_i - A_j)^2
+    real sA = real(0), sB = real(0);
+    const int ks[4] = {1, -1, 2, -2};
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      const real dx1 = p1 - T(0, 0, ks[s]), dx2 = p2 - T(1, 0, ks[s]), dxa = A2 - T(3, 0, ks[s]);
+      const real dy1 = p1 - T(0, ks[s], 0), dy2 = p2 - T(1, ks[s], 0), dya = A1 - T(2, ks[s], 0);
+      const real t = ((dx1 * dx1 + dx2 * dx2) + dxa * dxa) + ((dy1 * dy1 + dy2 * dy2) + dya * dya);
+      if (s < 2) sA += t; else sB += t;
+    }
+    e = (real(0.5) * AA * rho + real(0.125) * p.lambda * (real(1) - rho) * (real(1) - rho)) +
+        (p.jA * sA + p.jB * sB) -
+        real(0.5) * p.i12h * (p1 * (Sx2 + Sy2) - p2 * (Sx1 + Sy1)) +
+        real(0.5) * ii * (A2 * xyA1 + A1 * xyA2);
+    q = real(0.15915494309189535) * p.i12h * (dxA2 - dyA1);
   }
 
   __device__ __forceinline__ static void project_field(real*) {}
