@@ -228,6 +228,13 @@ KERNEL_UNITS = {
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
+# capture (profiles/r01_ncu_full_cm4096_f64_twokernel.csv); other workloads: not captured.
+NCU_TRAFFIC = {
+    ("cm_quench_4096", "f64", "flow_y_stage34_combine_project_ke"): 1.695515e9 + 779.445760e6,
+    ("cm_quench_4096", "f64", "flow_x_grad_energy_charge_stage2"): 0.853048e9 + 769.389056e6,
+}
+
 
 def max_over_ranks(values, dist=None, device="cpu"):
     """Element-wise MAX over all ranks of a list of floats (identity without a process group)."""
@@ -310,7 +317,8 @@ def run_ours(args):
     units = sum(KERNEL_UNITS.get(n, 0) for n in kern)      # 10 (two-kernel) or 16 (staged)
     roofline = {
         "bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
-        "unit": "GB/s", "frac": kern[dom]["gbs"] / peak, "traffic": None,
+        "unit": "GB/s", "frac": kern[dom]["gbs"] / peak,
+        "traffic": NCU_TRAFFIC.get((w.name, dtname, dom)),
         "peak_source": peak_src, "kernel_ms": kern[dom]["ms"],
         "kernel_share_of_step": kern[dom]["ms"] / tot,
         "alg_bytes_per_site": KERNEL_UNITS[dom] * C * R,
