@@ -64,7 +64,7 @@ enum { SS_RK4 = 0 };
 typedef struct {
   int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
                            /* reductions, E, Q, KE and the arrest test are always fp64      */
-  int batch;               /* >= 1 independent lattices sharing Nx, Ny, h, dt               */
+  int batch;               /* 1..65535 independent lattices sharing Nx, Ny, h, dt           */
   double dt;               /* <= 0 -> 0.5*h (Courant number C = 0.5)          */
   double kappa, B, K;      /* chiral magnet: DMI, Zeeman field, uniaxial anisotropy         */
   const double* B_batch;   /* optional HOST array[batch]: per-lattice B (overrides B)       */

@@ -46,7 +46,7 @@ bool valid_shape(int theory, int Nx, int Ny, const ss_params* p) {
   if (!p) return false;
   if (theory != SS_THEORY_CHIRAL_MAGNET && theory != SS_THEORY_ABELIAN_HIGGS) return false;
   if (p->dtype != SS_F64 && p->dtype != SS_F32) return false;
-  if (Nx < 5 || Ny < 5 || p->batch < 1) return false;
+  if (Nx < 5 || Ny < 5 || p->batch < 1 || p->batch > 65535) return false;  // grid.z
   if (p->dtype == SS_F64 ? (Nx % 2 != 0) : (Nx % 4 != 0)) return false;
   if (Nx > 16384 || Ny > 32768) return false;  // reduction tree limits (32 lanes x 8, 1024 x 32)
   if (p->arrest_log_capacity < 0) return false;
