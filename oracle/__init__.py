@@ -60,6 +60,7 @@ def lib():
         L.orc_flow_destroy.argtypes = [C.c_void_p]
         L.orc_flow_set.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_flow_step.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_flow_step_verlet.argtypes = [C.c_void_p, C.c_int64]
         L.orc_flow_get.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_flow_scalars.argtypes = [C.c_void_p, _dp, _dp, _dp, C.POINTER(C.c_int64),
                                        C.POINTER(C.c_int64), C.POINTER(C.c_int),
@@ -149,7 +150,10 @@ def accel(m, f):
 class Flow:
     """Arrested Newton flow on host arrays [C][Ny][Nx]."""
 
-    def __init__(self, m, dt=0.0):
+    def __init__(self, m, dt=0.0, integrator="rk4"):
+        """integrator: "rk4" or "verlet" (one gradient per step, DESIGN R15)."""
+        assert integrator in ("rk4", "verlet")
+        self.integrator = integrator
         self.m = m
         self.shape = (ncomp(m.theory), m.Ny, m.Nx)
         self._h = lib().orc_flow_create(C.byref(m), float(dt))
@@ -166,7 +170,10 @@ class Flow:
         lib().orc_flow_set(self._h, _p(phi), _p(vel))
 
     def step(self, k=1):
-        lib().orc_flow_step(self._h, int(k))
+        if self.integrator == "rk4":
+            lib().orc_flow_step(self._h, int(k))
+        else:
+            lib().orc_flow_step_verlet(self._h, int(k))
 
     def get_fields(self):
         phi, vel = np.empty(self.shape), np.empty(self.shape)

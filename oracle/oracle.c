@@ -601,6 +601,68 @@ void orc_flow_step(orc_flow* s, int64_t k) {
   free(ke);
 }
 
+/* One-gradient-per-step variant (PAPER.md:123 allows any "standard explicit time integrator
+ * such as" RK4; DESIGN R15): velocity Verlet for phi'' = -grad E with the same projection
+ * (PAPER.md:129+154) and the same arrest (eq. 4):
+ *   vh = arrested ? 0 : v
+ *   w    = vh + dt/2 a(phi)                      half kick  (a(phi) is s->a1, from flow_evaluate)
+ *   phi' = R(phi + dt w)                         drift + constraint
+ *   u    = w + dt/2 a(phi')                      half kick with the new acceleration
+ *   v'   = u - (u.phi')phi' (CM) | u (AH)
+ * then flow_evaluate on phi' (a1, E, Q, arrest).  One stencil pass per step. */
+void orc_flow_step_verlet(orc_flow* s, int64_t k) {
+  const int Nx = s->m.Nx, Ny = s->m.Ny, C = s->C;
+  const double dt = s->dt, h = s->m.h, hdt = 0.5 * dt;
+  double* ke = (double*)malloc(s->P * sizeof(double));
+  for (int64_t it = 0; it < k; ++it) {
+    memcpy(s->s, s->phi, C * s->P * sizeof(double)); /* frozen halo */
+#pragma omp parallel for schedule(static)
+    for (int j = 2; j < Ny - 2; ++j)
+      for (int i = 2; i < Nx - 2; ++i) {
+        double mm[4];
+        for (int c = 0; c < C; ++c) {
+          size_t a = at(Nx, Ny, c, j, i);
+          double vh = s->v_is_zero ? 0.0 : s->vel[a];
+          double w = vh + hdt * s->a1[a];
+          s->a2[a] = w; /* scratch: the half-kicked velocity */
+          mm[c] = s->phi[a] + dt * w;
+        }
+        if (s->m.theory == ORC_CM) {
+          double nn = sqrt((mm[0] * mm[0] + mm[1] * mm[1]) + mm[2] * mm[2]);
+          for (int c = 0; c < 3; ++c) mm[c] = mm[c] / nn;
+        }
+        for (int c = 0; c < C; ++c) s->s[at(Nx, Ny, c, j, i)] = mm[c];
+      }
+    orc_accel(&s->m, s->s, s->a4);
+    memset(ke, 0, s->P * sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (int j = 2; j < Ny - 2; ++j)
+      for (int i = 2; i < Nx - 2; ++i) {
+        double f[4], u[4];
+        for (int c = 0; c < C; ++c) {
+          size_t a = at(Nx, Ny, c, j, i);
+          f[c] = s->s[a];
+          u[c] = s->a2[a] + hdt * s->a4[a];
+        }
+        if (s->m.theory == ORC_CM) {
+          double un = (u[0] * f[0] + u[1] * f[1]) + u[2] * f[2];
+          for (int c = 0; c < 3; ++c) u[c] = u[c] - un * f[c];
+        }
+        double v2 = 0.0;
+        for (int c = 0; c < C; ++c) {
+          s->phi[at(Nx, Ny, c, j, i)] = f[c];
+          s->vel[at(Nx, Ny, c, j, i)] = u[c];
+          v2 += u[c] * u[c];
+        }
+        ke[(size_t)j * Nx + i] = 0.5 * v2;
+      }
+    s->KE = (h * h) * orc_tree_sum2d(ke, Nx, Ny);
+    s->n += 1;
+    flow_evaluate(s);
+  }
+  free(ke);
+}
+
 void orc_flow_get(const orc_flow* s, double* phi, double* vel) {
   if (phi) memcpy(phi, s->phi, s->C * s->P * sizeof(double));
   if (vel) {
