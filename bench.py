@@ -56,6 +56,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--staged", action="store_true", help="one kernel per RK4 stage (A/B)")
+    ap.add_argument("--integrator", default="rk4", choices=["rk4", "verlet"],
+                    help="rk4 = the metric's flow step (default); verlet = SURVEY 8(f) NEXT-1")
     ap.add_argument("--cps", type=int, default=0, help="chunks per segment (0 = auto)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0,
                     help="target CPU time of the oracle sample")
@@ -136,14 +138,14 @@ def nvml_index(torch, dev):
         return dev.index or 0
 
 
-def time_oracle(w, seconds, lattices=None):
+def time_oracle(w, seconds, lattices=None, integrator="rk4"):
     """Oracle as it stands on this box's host cores: one untimed step, then as many steps as fit
     in about `seconds` (at least 1) on lattice 0 (and only lattice 0 of a batched workload)."""
     import oracle
     b = 0
     B = w.B if w.B_batch is None else float(w.B_batch[b])
     fl = oracle.Flow(oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K,
-                                  lam=w.lam), w.dt)
+                                  lam=w.lam), w.dt, integrator=integrator)
     fl.set_fields(w.fields[b])
     t0 = time.perf_counter()
     fl.step(1)
@@ -184,13 +186,13 @@ def run_reference(args):
     w, _ = make_workload(args.workload)
     full = min(w.Nx, w.Ny)
     cal = crop_workload(w, min(256, full))
-    rate = time_oracle(cal, 0.0)["value"]                     # site-updates/s, 1 step
+    rate = time_oracle(cal, 0.0, integrator=args.integrator)["value"]                     # site-updates/s, 1 step
     budget = 120.0 / max(1, args.steps + args.warmup)
     S = int((rate * budget) ** 0.5) // 64 * 64
     S = max(64, min(full, S))
     c = crop_workload(w, S)
     fl = oracle.Flow(oracle.model(c.theory, S, S, c.h, kappa=c.kappa, B=c.B, K=c.K, lam=c.lam),
-                     c.dt)
+                     c.dt, integrator=args.integrator)
     fl.set_fields(c.fields[0])
     fl.step(args.warmup)
     t0 = time.perf_counter()
@@ -220,6 +222,8 @@ KERNEL_UNITS = {
     # two-kernel schedule (default)
     "flow_y_stage34_combine_project_ke": 6,   # reads phi, v, a1, a2 -> writes phi', v'
     "flow_x_grad_energy_charge_stage2": 4,    # reads phi', v'       -> writes a1, a2 (+ E, Q partials)
+    # one-gradient-per-step integrator (--integrator verlet): reads phi, v, a -> phi', v', a'
+    "flow_v_verlet_step_energy_charge_ke": 6,
     # one kernel per RK4 stage (--staged, the first round-1 schedule)
     "stage2": 3,                       # reads phi, v            -> writes a2
     "stage3": 4,                       # reads phi, v, a1        -> writes a3
@@ -273,7 +277,8 @@ def run_ours(args):
     R = 8 if dtname == "f64" else 4
     host = torch.from_numpy(w.fields).to(tdt).contiguous().pin_memory()
     s = ss.solver_for(w, dtype=dtype, device=str(dev), cps=args.cps,
-                      flags=ss.FLAG_STAGED if args.staged else 0)
+                      flags=ss.FLAG_STAGED if args.staged else 0,
+                      integrator=ss.VERLET if args.integrator == "verlet" else ss.RK4)
     s.set_fields(host.to(dev))
     sites = w.interior_sites
     field_bytes = host.numel() * R
@@ -388,7 +393,7 @@ def main():
     w = r["w"]
     cpu = None
     if r["rank"] == 0 and r["world"] == 1 and not args.no_cpu_baseline:
-        cpu = time_oracle(w, args.cpu_seconds)
+        cpu = time_oracle(w, args.cpu_seconds, integrator=args.integrator)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
     bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"} & set(r["clocks"]["reasons"])
     line = {
@@ -399,7 +404,7 @@ def main():
         "config": {"workload": w.name, "theory": "chiral_magnet" if w.theory == 0 else
                    "abelian_higgs", "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
                    "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
-                   "integrator": "rk4", "schedule": "staged" if args.staged else "two-kernel",
+                   "integrator": args.integrator, "schedule": "staged" if args.staged else "two-kernel",
                    "parallelism": f"replicas x{r['world']}",
                    "l2_policy": "working set (7 field arrays) larger than L2; no flush needed"
                    if 7 * r["field_bytes"] > 3 * 126e6 else

@@ -58,8 +58,11 @@ enum {
   SS_ERR_NONFINITE = -6    /* an energy became NaN/Inf (values are still written)           */
 };
 
-/* Integrators.  SS_RK4 is the paper's; others are reserved. */
-enum { SS_RK4 = 0 };
+/* Integrators.  SS_RK4 is the paper's example ("such as fourth-order Runge-Kutta").
+ * SS_VERLET is the one-gradient-per-step variant (DESIGN R15): velocity Verlet
+ *   w = vh + dt/2 a(phi), phi' = R(phi + dt w), v' = Pi(w + dt/2 a(phi'))
+ * with the same projection (PAPER.md:129+154) and the same arrest (eq. 4). */
+enum { SS_RK4 = 0, SS_VERLET = 1 };
 
 typedef struct {
   int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
@@ -74,7 +77,7 @@ typedef struct {
   void* stream;            /* cudaStream_t owned by the caller; NULL = default stream       */
   int64_t arrest_log_capacity; /* entries per lattice; 0 -> 4096; later arrests are counted */
                                /* but not logged                                            */
-  int integrator;          /* SS_RK4                                                        */
+  int integrator;          /* SS_RK4 | SS_VERLET                                            */
   int flags;               /* bit 0: launch kernels one by one instead of replaying the     */
                            /* per-step CUDA graph (debugging; same results)                 */
                            /* bit 1: one kernel per RK4 stage (the round-1 schedule, kept   */

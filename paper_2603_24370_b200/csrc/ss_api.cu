@@ -117,7 +117,8 @@ struct ss_solver {
   int flags;
   bool fields_set;
   int cur;  // which ping-pong buffer holds (phi, v)
-  int cps[2];  // chunks per y-segment of flow kernels X, Y
+  int cps[3];  // chunks per y-segment of flow kernels X, Y, V
+  int integrator;
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
@@ -230,7 +231,9 @@ bool make_tmap(const ss_solver* s, void* base, CUtensorMap* out) {
 
 template <int THEORY, typename real>
 void* flow_func_t(int kind) {
-  return kind == KX ? (void*)flow_kernel<THEORY, real, KX> : (void*)flow_kernel<THEORY, real, KY>;
+  return kind == KX   ? (void*)flow_kernel<THEORY, real, KX>
+         : kind == KY ? (void*)flow_kernel<THEORY, real, KY>
+                      : (void*)flow_kernel<THEORY, real, KV>;
 }
 void* flow_func(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
@@ -242,7 +245,9 @@ void* flow_func(int theory, int dtype, int kind) {
 }
 template <int THEORY, typename real>
 int flow_smem_t(int kind) {
-  return kind == KX ? FlowCfg<THEORY, real, KX>::SMEM : FlowCfg<THEORY, real, KY>::SMEM;
+  return kind == KX   ? FlowCfg<THEORY, real, KX>::SMEM
+         : kind == KY ? FlowCfg<THEORY, real, KY>::SMEM
+                      : FlowCfg<THEORY, real, KV>::SMEM;
 }
 int flow_smem(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
@@ -255,7 +260,9 @@ int flow_smem(int theory, int dtype, int kind) {
 
 template <int THEORY, typename real>
 int flow_threads_t(int kind) {
-  return kind == KX ? FlowCfg<THEORY, real, KX>::THREADS : FlowCfg<THEORY, real, KY>::THREADS;
+  return kind == KX   ? FlowCfg<THEORY, real, KX>::THREADS
+         : kind == KY ? FlowCfg<THEORY, real, KY>::THREADS
+                      : FlowCfg<THEORY, real, KV>::THREADS;
 }
 int flow_threads(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
@@ -266,18 +273,22 @@ int flow_threads(int theory, int dtype, int kind) {
   return dtype == SS_F64 ? flow_threads_t<kAH, double>(kind) : flow_threads_t<kAH, float>(kind);
 }
 
-// kernel X (kind KX) evaluates the state in buffer `in`; kernel Y advances `in` -> `in ^ 1`
+// kernel X (kind KX) evaluates the state in buffer `in`; kernels Y and V advance `in` -> `in ^ 1`
+// (V also a: acc(in) -> acc(in ^ 1))
 template <typename real>
 bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   FlowArgs<real> a;
   memset(&a, 0, sizeof(a));
   const double dt = s->dt, h = s->h;
   if (!make_tmap(s, s->phi(in), &a.tm[0]) || !make_tmap(s, s->vel(in), &a.tm[1]) ||
-      !make_tmap(s, s->acc(0), &a.tm[2]) || !make_tmap(s, s->acc(1), &a.tm[3]))
+      !make_tmap(s, s->acc(kind == KV ? in : 0), &a.tm[2]) || !make_tmap(s, s->acc(1), &a.tm[3]))
     return false;
   if (kind == KX) {
     a.out0 = (real*)s->acc(0); a.out1 = (real*)s->acc(1);
     a.part0 = s->part(0); a.part1 = s->part(1);
+  } else if (kind == KV) {
+    a.out0 = (real*)s->phi(in ^ 1); a.out1 = (real*)s->vel(in ^ 1); a.out2 = (real*)s->acc(in ^ 1);
+    a.part0 = s->part(0); a.part1 = s->part(1); a.part2 = s->part(2);
   } else {
     a.out0 = (real*)s->phi(in ^ 1); a.out1 = (real*)s->vel(in ^ 1);
     a.part0 = s->part(2); a.part1 = nullptr;
@@ -305,7 +316,9 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   n.block = dim3(flow_threads(s->theory, s->dtype, kind), 1, 1);
   n.smem = (size_t)flow_smem(s->theory, s->dtype, kind);
   n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
-  n.name = kind == KX ? "flow_x_grad_energy_charge_stage2" : "flow_y_stage34_combine_project_ke";
+  n.name = kind == KX   ? "flow_x_grad_energy_charge_stage2"
+           : kind == KY ? "flow_y_stage34_combine_project_ke"
+                        : "flow_v_verlet_step_energy_charge_ke";
   *out = n;
   return true;
 }
@@ -414,7 +427,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (!out) return SS_ERR_ARG;
   *out = nullptr;
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
-  if (p->integrator != SS_RK4) return SS_ERR_UNSUPPORTED;
+  if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
+  if (p->integrator == SS_VERLET && (p->flags & 2)) return SS_ERR_UNSUPPORTED;
   int ndev = 0;
   if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
     if (ndev == 0) snprintf(g_cuda_msg, sizeof(g_cuda_msg), "no CUDA device (libss has no CPU path)");
@@ -435,6 +449,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->L = L;
   s->log_cap = p->arrest_log_capacity > 0 ? p->arrest_log_capacity : 4096;
   s->flags = p->flags;
+  s->integrator = p->integrator;
   s->fields_set = false;
   s->cur = 0;
   s->steps_done = 0; s->launches = 0;
@@ -460,7 +475,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     int sms = 148, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    for (int kind = 0; kind < 2; ++kind) {
+    for (int kind = 0; kind < 3; ++kind) {
       void* f = flow_func(theory, p->dtype, kind);
       const int smem = flow_smem(theory, p->dtype, kind);
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -483,6 +498,14 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       st.push_back(make_stage_node(s, 4, cur));
       st.push_back(make_stage_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
       ev.push_back(make_stage_node(s, 1, cur));
+    } else if (s->integrator == SS_VERLET) {
+      KernelNode v, x0;
+      if (!make_flow_node(s, KV, cur, &v) || !make_flow_node(s, KX, cur, &x0)) {
+        ss_destroy(s);
+        return SS_ERR_CUDA;
+      }
+      st.push_back(v);   // the whole step: phi', v', a', E, Q, KE
+      ev.push_back(x0);  // a (-> acc(0), only used with cur == 0), E, Q
     } else {
       KernelNode y, x, x0;
       if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, KX, cur ^ 1, &x) ||

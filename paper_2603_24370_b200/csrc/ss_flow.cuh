@@ -8,6 +8,9 @@
 //       phi3 = R((phi + dt/2 vh) + dt^2/4 a1), a3 = -Pi G(phi3)
 //       phi4 = R((phi + dt vh) + dt^2/2 a2),   a4 = -Pi G(phi4)
 //       RK4 combine + projections (PAPER.md:123, :129+154), vh = arrested ? 0 : v (eq. 4)
+//   flow_kernel<THEORY, real, KV>  "V": the whole one-gradient-per-step (velocity Verlet, DESIGN
+//       R15) step: reads phi, v, a -> writes phi', v', a', E/Q/KE partials
+//       w = vh + dt/2 a, phi' = R(phi + dt w), a' = -Pi G(phi'), v' = Pi(w + dt/2 a')
 //
 // A CTA owns a strip of FW = 64 columns and a segment of rows, and marches down the segment in
 // chunks of FR = 4 rows; a thread owns SPT vertically adjacent sites of the chunk.  Per chunk f
@@ -30,15 +33,17 @@ namespace ss {
 constexpr int FW = SEG;             // strip width = row segment of the reduction tree
 constexpr int FR = 4;               // rows per chunk
 constexpr int FWP = FW + 2 * HALO;  // ring width
-constexpr int KX = 0, KY = 1;
+constexpr int KX = 0, KY = 1, KV = 2;
 
 template <typename real>
 struct FlowArgs {
-  alignas(64) CUtensorMap tm[4];  // phi, v, a1, a2 as (x, y, batch*C) tensors
-  real* out0;                     // X: a1    Y: phi'
-  real* out1;                     // X: a2    Y: v'
-  double* part0;                  // X: e     Y: ke     [batch][Ny][nseg]
-  double* part1;                  // X: q
+  alignas(64) CUtensorMap tm[4];  // phi, v, a1 (V: a), a2 as (x, y, batch*C) tensors
+  real* out0;                     // X: a1    Y, V: phi'
+  real* out1;                     // X: a2    Y, V: v'
+  real* out2;                     //          V: a'
+  double* part0;                  // X, V: e  Y: ke     [batch][Ny][nseg]
+  double* part1;                  // X, V: q
+  double* part2;                  // V: ke
   const LatticeState* state;
   const double* Bb;               // [batch] Zeeman field per lattice
   int Nx, Ny, nseg, cps;          // cps = chunks per segment
@@ -113,24 +118,25 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 template <int THEORY, typename real, int KIND>
 struct FlowCfg {
   static constexpr int C = TheoryOf<THEORY, real>::type::C;
-  static constexpr int SPT = KIND == KX ? SS_SPT_X : SS_SPT_Y;
+  static constexpr int SPT = KIND == KY ? SS_SPT_Y : SS_SPT_X;
   static constexpr int ROWT = FR / SPT;                          // thread rows
   static constexpr int THREADS = FW * ROWT;
-  static constexpr int RING = KIND == KX ? SS_RING_X : SS_RING_Y;
-  static constexpr int NST = KIND == KX ? SS_NST_X : SS_NST_Y;
+  static constexpr int RING = KIND == KY ? SS_RING_Y : SS_RING_X;
+  static constexpr int NST = KIND == KY ? SS_NST_Y : SS_NST_X;
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
   static constexpr int RAWW = FW + 2 * XPAD;                     // staged width (>= FWP)
   static constexpr int BOXB = C * FR * RAWW * (int)sizeof(real); // bytes one TMA box delivers
   static constexpr int ARRB = (BOXB + 127) / 128 * 128;          // 128-byte aligned slot
-  static constexpr int NARR = KIND == KX ? 2 : 4;                // phi, v (, a1, a2)
+  static constexpr int NARR = KIND == KX ? 2 : (KIND == KY ? 4 : 3);  // phi, v (, a1 (, a2))
+  static constexpr int NRING = KIND == KV ? 1 : 2;
   static constexpr int STAGEB = NARR * ARRB;
   static constexpr int OFF_RING = NST * STAGEB;
   static constexpr int RP = RING * FWP;                          // elements of one ring plane
   static constexpr int RINGN = C * RP;                           // elements of one ring
-  static constexpr int OFF_RED = OFF_RING + 2 * RINGN * (int)sizeof(real);
-  static constexpr int OFF_BAR = OFF_RED + 2 * 2 * FR * 2 * (int)sizeof(double);
+  static constexpr int OFF_RED = OFF_RING + NRING * RINGN * (int)sizeof(real);
+  static constexpr int OFF_BAR = OFF_RED + 2 * 3 * FR * 2 * (int)sizeof(double);
   static constexpr int SMEM = OFF_BAR + NST * 8;
-  static constexpr int WANTB = KIND == KX ? SS_MINB_X : SS_MINB_Y;
+  static constexpr int WANTB = KIND == KY ? SS_MINB_Y : SS_MINB_X;
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
   static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTB ? FITB : WANTB);
   static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small for a single barrier");
@@ -157,11 +163,11 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   using Th = typename TheoryOf<THEORY, real>::type;
   using Cfg = FlowCfg<THEORY, real, KIND>;
   constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT, NST = Cfg::NST;
-  constexpr int NQ = KIND == KX ? 2 : 1;  // partial-sum quantities
+  constexpr int NQ = KIND == KX ? 2 : (KIND == KY ? 1 : 3);  // partial-sum quantities
   extern __shared__ __align__(128) unsigned char smem[];
-  real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3
-  real* ringB = ringA + Cfg::RINGN;                             // X: phi2   Y: phi4
-  double* red = reinterpret_cast<double*>(smem + Cfg::OFF_RED); // [2 parity][2 q][FR][2 halves]
+  real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3   V: phi'
+  real* ringB = ringA + (Cfg::NRING - 1) * Cfg::RINGN;          // X: phi2   Y: phi4
+  double* red = reinterpret_cast<double*>(smem + Cfg::OFF_RED); // [2 parity][3 q][FR][2 halves]
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + Cfg::OFF_BAR);
 
   const int tid = threadIdx.x;
@@ -171,7 +177,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   const int NC = (Ny + FR - 1) / FR;
   const int cs = blockIdx.y * p.cps, ce = min(cs + p.cps, NC);  // stencil chunks [cs, ce)
   const int f0 = max(cs - 1, 0), f1 = min(ce, NC - 1);          // fill chunks [f0, f1]
-  const bool vz = KIND == KY ? (p.state[b].v_is_zero != 0) : false;
+  const bool vz = KIND != KX ? (p.state[b].v_is_zero != 0) : false;
   const real Bz = real(p.Bb[b]);
 
   if (tid == 0) {
@@ -185,11 +191,11 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   auto issue = [&](int f) {
     unsigned char* st = smem + ((f - f0) % NST) * Cfg::STAGEB;
     uint64_t* bar = &full[(f - f0) % NST];
-    const int narr = KIND == KX ? 2 : (vz ? 2 : 4);
+    const int narr = KIND == KX ? 2 : (KIND == KY ? (vz ? 2 : 4) : (vz ? 2 : 3));
     mbar_expect_tx(bar, (uint32_t)(narr * Cfg::BOXB));
 #pragma unroll
     for (int a = 0; a < Cfg::NARR; ++a) {
-      if (KIND == KY && vz && (a == 1 || a == 3)) continue;
+      if (KIND != KX && vz && (a == 1 || a == 3)) continue;
       tma_load_3d(st + a * Cfg::ARRB, &p.tm[a], x0 - Cfg::XPAD, f * FR, b * C, bar);
     }
   };
@@ -220,6 +226,16 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 #pragma unroll
         for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * rvel[c * FR * RW + ro];
         Th::project_field(Bf);
+      } else if (KIND == KV) {
+        const real* ra = reinterpret_cast<const real*>(st + 2 * Cfg::ARRB);
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          const real vh = vz ? real(0) : rvel[c * FR * RW + ro];
+          const real w = vh + p.hdt * ra[c * FR * RW + ro];
+          A[c] = A[c] + p.dt * w;
+          if (keep) keep[c] = w;
+        }
+        Th::project_field(A);
       } else {
         const real* ra1 = reinterpret_cast<const real*>(st + 2 * Cfg::ARRB);
         const real* ra2 = reinterpret_cast<const real*>(st + 3 * Cfg::ARRB);
@@ -245,7 +261,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 #pragma unroll
     for (int c = 0; c < C; ++c) {
       ringA[c * RP + wo] = A[c];
-      ringB[c * RP + wo] = Bf[c];
+      if (KIND != KV) ringB[c * RP + wo] = Bf[c];
     }
   };
 
@@ -254,8 +270,8 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     if (tid < NQ * FR) {
       const int q = tid / FR, row = tid % FR, gy = sc * FR + row;
       if (gy < Ny) {
-        const double* rr = red + ((par * 2 + q) * FR + row) * 2;
-        double* dst = q == 0 ? p.part0 : p.part1;
+        const double* rr = red + ((par * 3 + q) * FR + row) * 2;
+        double* dst = q == 0 ? p.part0 : (q == 1 ? p.part1 : p.part2);
         dst[((long long)b * Ny + gy) * p.nseg + blockIdx.x] = rr[0] + rr[1];
       }
     }
@@ -288,12 +304,12 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       int rw[SPT + 4];
 #pragma unroll
       for (int j = 0; j < SPT + 4; ++j) rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
-      double s0[SPT], s1[SPT];
+      double s0[SPT], s1[SPT], s2[SPT];
       bool act[SPT];
       real aA[SPT][C];
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
-        s0[k] = s1[k] = 0.0;
+        s0[k] = s1[k] = s2[k] = 0.0;
         act[k] = xin && gy0 + k >= HALO && gy0 + k < Ny - HALO;
       }
       const long long o = (long long)b * C * p.plane + (long long)gy0 * Nx + gx;
@@ -314,7 +330,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
           auto TA = [&](int c, int dy, int dx) -> real {
             return dx == 0 ? col[c][k + dy + 2] : ringA[c * RP + rw[k + dy + 2] + dx];
           };
-          if (KIND == KX) {
+          if (KIND == KX || KIND == KV) {
             real e, q;
             if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
               Th::accel(TA, p, Bz, aA[k]);
@@ -322,23 +338,44 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
             } else {
               Th::accel_densities_bulk(TA, p, Bz, aA[k], e, q);
             }
-#pragma unroll
-            for (int c = 0; c < C; ++c) o0[c * p.plane + k * Nx] = aA[k][c];
             s0[k] = double(e);
             s1[k] = double(q);
+            if (KIND == KX) {
+#pragma unroll
+              for (int c = 0; c < C; ++c) o0[c * p.plane + k * Nx] = aA[k][c];
+            } else {  // second half kick, tangent projection, KE
+              real fn[C], u[C];
+#pragma unroll
+              for (int c = 0; c < C; ++c) {
+                fn[c] = col[c][k + 2];
+                u[c] = keep_old[k][c] + p.hdt * aA[k][c];
+              }
+              Th::project_velocity(u, fn);
+              real v2 = real(0);
+#pragma unroll
+              for (int c = 0; c < C; ++c) {
+                o0[c * p.plane + k * Nx] = fn[c];
+                o1[c * p.plane + k * Nx] = u[c];
+                p.out2[o + c * p.plane + k * Nx] = aA[k][c];
+                v2 += u[c] * u[c];
+              }
+              s2[k] = 0.5 * double(v2);
+            }
           } else {
             Th::accel(TA, p, Bz, aA[k]);
           }
         }
       }
       // ---- ring B (X: phi2 -> a2    Y: phi4 -> a4, RK4 combine, projections, KE)
+      if (KIND != KV) {
 #pragma unroll
-      for (int c = 0; c < C; ++c)
+        for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringB[c * RP + rw[j]];
+          for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringB[c * RP + rw[j]];
+      }
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
-        if (act[k]) {
+        if (KIND != KV && act[k]) {
           auto TB = [&](int c, int dy, int dx) -> real {
             return dx == 0 ? col[c][k + dy + 2] : ringB[c * RP + rw[k + dy + 2] + dx];
           };
@@ -371,10 +408,14 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       // segment are added (low + high) by flush_partials after the next barrier
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
-        double* rr = red + (((f & 1) * 2) * FR + r0 + k) * 2 + (tx >> 5);
-        if (KIND == KX) {
+        double* rr = red + (((f & 1) * 3) * FR + r0 + k) * 2 + (tx >> 5);
+        if (KIND == KX || KIND == KV) {
           const double t = warp_tree2(s0[k], s1[k], lane);
           if (lane < 2) rr[lane * FR * 2] = t;
+          if (KIND == KV) {
+            const double t2 = warp_tree(s2[k]);
+            if (lane == 0) rr[2 * FR * 2] = t2;
+          }
         } else {
           const double t = warp_tree(s0[k]);
           if (lane == 0) rr[0] = t;

@@ -23,6 +23,7 @@ THEORY_CHIRAL_MAGNET, THEORY_ABELIAN_HIGGS = 0, 1
 F64, F32 = 0, 1
 OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE = \
     0, -1, -2, -3, -4, -5, -6
+RK4, VERLET = 0, 1
 FLAG_NO_GRAPH = 1
 FLAG_STAGED = 2
 
@@ -84,7 +85,7 @@ def _check(rc, where, allow=()):
     return rc
 
 
-def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0):
+def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, integrator=0):
     p = ss_params()
     p.dtype, p.batch, p.dt = int(dtype), int(batch), float(dt)
     p.kappa, p.B, p.K, p.lam = float(kappa), float(B), float(K), float(lam)
@@ -93,7 +94,7 @@ def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0):
         keep = (C.c_double * int(batch))(*[float(x) for x in B_batch])
         p.B_batch = C.cast(keep, _dp)
     p.arrest_log_capacity = int(log_cap)
-    p.integrator, p.flags = 0, int(flags)
+    p.integrator, p.flags = int(integrator), int(flags)
     p.chunks_per_segment = int(cps)
     return p, keep
 
@@ -107,7 +108,8 @@ class Solver:
     """ss_create ... ss_destroy around torch-owned device memory and the current torch stream."""
 
     def __init__(self, theory, Nx, Ny, h, *, dtype=F64, batch=1, dt=0.0, kappa=0.0, B=0.0, K=0.0,
-                 lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, device="cuda:0", stream=None):
+                 lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, integrator=RK4, device="cuda:0",
+                 stream=None):
         self.theory, self.Nx, self.Ny, self.batch = int(theory), int(Nx), int(Ny), int(batch)
         self.C = 3 if theory == THEORY_CHIRAL_MAGNET else 4
         self.dtype = dtype
@@ -115,7 +117,8 @@ class Solver:
         self.torch_dtype = torch.float64 if dtype == F64 else torch.float32
         self.device = torch.device(device)
         self._h = C.c_void_p()
-        p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps)
+        p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps,
+                          integrator)
         nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
         if nbytes == 0:
             raise SSError(ERR_ARG, "ss_workspace_bytes")
@@ -225,8 +228,9 @@ class Solver:
         return _lib.ss_launch_count(self._h)
 
 
-def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0) -> Solver:
+def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0,
+               integrator=RK4) -> Solver:
     """Solver configured from a workloads.Workload (sizes and parameters only)."""
     return Solver(w.theory, w.Nx, w.Ny, w.h, dtype=dtype, batch=w.batch, dt=w.dt, kappa=w.kappa,
                   B=w.B, K=w.K, lam=w.lam, B_batch=w.B_batch, log_cap=log_cap, flags=flags,
-                  cps=cps, device=device)
+                  cps=cps, integrator=integrator, device=device)

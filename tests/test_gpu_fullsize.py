@@ -23,9 +23,9 @@ def _floor(m, phi, E):
     return max(abs(E), m.h * m.h * float(np.abs(de).sum()), 1e-300)
 
 
-def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11):
+def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4"):
     ss = _ss()
-    s = ss.solver_for(w)
+    s = ss.solver_for(w, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
     s.set_fields(torch.from_numpy(w.fields).to("cuda:0"))
     s.step(steps)
     phi, vel = s.get_fields()
@@ -35,7 +35,7 @@ def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11):
     for b in lattices:
         B = w.B if w.B_batch is None else float(w.B_batch[b])
         m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam)
-        fl = oracle.Flow(m, w.dt)
+        fl = oracle.Flow(m, w.dt, integrator=integrator)
         fl.set_fields(w.fields[b])
         fl.step(steps)
         ophi, ovel = fl.get_fields()
@@ -63,6 +63,10 @@ def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11):
 
 def test_config4_cm_4096_fp64_full_size():
     _check(W.baseline_config(4), steps=3)
+
+
+def test_config4_cm_4096_full_size_verlet():
+    _check(W.baseline_config(4), steps=4, integrator="verlet")
 
 
 def test_config2_cm_1024_full_size():

@@ -38,14 +38,15 @@ def _dev(a, dtype=torch.float64):
     return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0", dtype=dtype).contiguous()
 
 
-def _run_parity(w, checkpoints=CHECKPOINTS, flags=0, field_tol=1e-11, lattices=None):
+def _run_parity(w, checkpoints=CHECKPOINTS, flags=0, field_tol=1e-11, lattices=None,
+                integrator="rk4"):
     ss = _ss()
-    s = ss.solver_for(w, flags=flags)
+    s = ss.solver_for(w, flags=flags, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
     s.set_fields(_dev(w.fields))
     lattices = range(w.batch) if lattices is None else lattices
     flows = {}
     for b in lattices:
-        fl = oracle.Flow(_model(w, b), w.dt)
+        fl = oracle.Flow(_model(w, b), w.dt, integrator=integrator)
         fl.set_fields(w.fields[b])
         flows[b] = fl
     E0 = s.energy()
@@ -115,6 +116,52 @@ def test_batched_sweep_per_lattice_arrests():
     s, flows = _run_parity(w)
     logs = [tuple(s.arrests(b)[0]) for b in range(w.batch)]
     assert len(set(logs)) > 1            # different B -> different arrest histories
+
+
+def test_verlet_cm_ragged_first_100_steps_with_arrests():
+    # one-gradient-per-step integrator (DESIGN R15), same tolerances; config-1 recipe on a ragged
+    # lattice; the first arrests fall inside the window
+    w = W.cm_multi(N=250, count=3, margin=12.0, min_sep=14.0)
+    s, flows = _run_parity(w, integrator="verlet")
+    assert len(flows[0].arrests()) >= 1
+
+
+def test_verlet_ah_and_batched():
+    w = W.ah_vortices(N=150, h=0.1, lam=2.0, count=2, min_sep=2.0)
+    _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50), integrator="verlet")
+    w = W.cm_sweep(batch=5, N=96)
+    s, flows = _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50), integrator="verlet")
+    for Nx, Ny in ((6, 5), (8, 7)):
+        rng = np.random.default_rng(Nx * 10 + Ny)
+        f = rng.standard_normal((1, 3, Ny, Nx))
+        f /= np.sqrt((f * f).sum(1, keepdims=True))
+        w = W.Workload("tiny", W.CM, Nx, Ny, 0.2, 0.1, kappa=1.0, B=0.6, K=0.1, fields=f)
+        _run_parity(w, checkpoints=(1, 2, 5), integrator="verlet")
+
+
+def test_verlet_fp32_and_graph_vs_direct():
+    ss = _ss()
+    w = W.cm_single(N=64)
+    s = ss.solver_for(w, dtype=ss.F32, integrator=ss.VERLET)
+    s.set_fields(_dev(w.fields, torch.float32))
+    fl = oracle.Flow(_model(w), w.dt, integrator="verlet")
+    fl.set_fields(w.fields[0])
+    for _ in range(3):
+        s.step(100)
+        fl.step(100)
+        phi = fl.get_fields()[0]
+        assert abs(s.energy()[0] - fl.energy) <= 1e-4 * _floor(fl.m, phi, fl.energy)
+    outs = []
+    for flags in (0, ss.FLAG_NO_GRAPH):
+        s = ss.solver_for(w, flags=flags, integrator=ss.VERLET)
+        s.set_fields(_dev(w.fields))
+        s.step(41)
+        f, v = s.get_fields()
+        outs.append((f.cpu(), v.cpu(), s.energy(), s.charge(), s.arrests(0)))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    assert outs[0][2:] == outs[1][2:]
+    with pytest.raises(ss.SSError):
+        ss.solver_for(w, flags=ss.FLAG_STAGED, integrator=ss.VERLET)   # no staged Verlet
 
 
 def test_graph_and_direct_launch_agree_bitwise():
