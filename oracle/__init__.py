@@ -33,7 +33,7 @@ def build(force: bool = False) -> str:
 class _Model(C.Structure):
     _fields_ = [("theory", C.c_int), ("Nx", C.c_int), ("Ny", C.c_int), ("h", C.c_double),
                 ("kappa", C.c_double), ("B", C.c_double), ("K", C.c_double),
-                ("lam", C.c_double)]
+                ("lam", C.c_double), ("dmi", C.c_int), ("d", C.c_double * 6)]
 
 
 _lib = None
@@ -50,6 +50,8 @@ def lib():
         L.orc_tree_sum2d.restype = C.c_double
         L.orc_cm_energy_bond.argtypes = [_dp, C.c_int, C.c_int] + [C.c_double] * 4
         L.orc_cm_energy_bond.restype = C.c_double
+        L.orc_cm_energy_bond_d.argtypes = [_dp, C.c_int, C.c_int] + [C.c_double] * 4 + [_dp]
+        L.orc_cm_energy_bond_d.restype = C.c_double
         L.orc_ah_energy_bond.argtypes = [_dp, C.c_int, C.c_int, C.c_double, C.c_double]
         L.orc_ah_energy_bond.restype = C.c_double
         L.orc_energy_charge.argtypes = [C.POINTER(_Model), _dp, C.c_int, _dp, _dp, _dp, _dp]
@@ -90,9 +92,15 @@ def ncomp(theory: int) -> int:
     return 3 if theory == CM else 4
 
 
-def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0):
-    return _Model(int(theory), int(Nx), int(Ny), float(h), float(kappa), float(B), float(K),
-                  float(lam))
+def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None):
+    """dmi: None = kappa n.(curl n) (BASELINE), else the six numbers (d_x, d_y) of
+    PAPER.md:196 eq. (5): e_DMI = kappa sum_mu d_mu . (n x d_mu n)."""
+    m = _Model(int(theory), int(Nx), int(Ny), float(h), float(kappa), float(B), float(K),
+               float(lam))
+    if dmi is not None:
+        m.dmi = 1
+        m.d = (C.c_double * 6)(*[float(x) for x in np.asarray(dmi).reshape(6)])
+    return m
 
 
 def stencil(op: str, f, h):
@@ -118,6 +126,9 @@ def energy_bond(m, f):
     """Plain bond-sum definition of E_h (straight summation)."""
     f = _f64(f)
     if m.theory == CM:
+        if m.dmi:
+            d = np.array(list(m.d))
+            return lib().orc_cm_energy_bond_d(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K, _p(d))
         return lib().orc_cm_energy_bond(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K)
     return lib().orc_ah_energy_bond(_p(f), m.Nx, m.Ny, m.h, m.lam)
 

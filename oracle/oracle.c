@@ -221,6 +221,83 @@ static void cm_site_gradient(const double* n, int Nx, int Ny, int j, int i, doub
          2.0 * kappa * (Dx(n2, Nx, j, i, h) - Dy(n1, Nx, j, i, h)) - (B + 2.0 * K * n3[a]);
 }
 
+/* ---- general DMI (eq. (5): D sum_i d_i . (n x d_i n); DESIGN R16) -------------
+ * e_DMI = kappa sum_{mu=x,y} d_mu . (n x D_mu n) with two constant vectors d_x, d_y (d[0..2],
+ * d[3..5]).  BASELINE's kappa n.(curl n) is d_mu = -e_mu ("Bloch"); the functions above are
+ * that special case, written out, and stay the definition when the model carries no table.
+ * Discrete energy: the bond (i, j = i + k mu) carries  + 2 kappa h^2 c_k d_mu . (n_i x n_j);
+ * site form  w(j) kappa c_k d_mu . (n_i x n_j);  gradient  2 kappa sum_mu (D_mu n) x d_mu. */
+static inline double dot_cross(const double* d, double a1, double a2, double a3, double b1,
+                               double b2, double b3) { /* d . (a x b) */
+  return d[0] * (a2 * b3 - a3 * b2) + d[1] * (a3 * b1 - a1 * b3) + d[2] * (a1 * b2 - a2 * b1);
+}
+
+double orc_cm_energy_bond_d(const double* n, int Nx, int Ny, double h, double kappa, double B,
+                            double K, const double* d) {
+  const double *n1 = n, *n2 = n + (size_t)Nx * Ny, *n3 = n + 2 * (size_t)Nx * Ny;
+  double E = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t a = (size_t)j * Nx + i;
+      for (int mu = 0; mu < 2; ++mu)
+        for (int k = 1; k <= 2; ++k) {
+          int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+          if (!inside(Nx, Ny, i2, j2)) continue;
+          if (!interior(Nx, Ny, i, j) && !interior(Nx, Ny, i2, j2)) continue;
+          size_t b = (size_t)j2 * Nx + i2;
+          double dx1 = n1[a] - n1[b], dx2 = n2[a] - n2[b], dx3 = n3[a] - n3[b];
+          double ex = 0.5 * Jw[k] * (dx1 * dx1 + dx2 * dx2 + dx3 * dx3);
+          double cr = dot_cross(d + 3 * mu, n1[a], n2[a], n3[a], n1[b], n2[b], n3[b]);
+          E += ex + 2.0 * kappa * (h * h) * cw(k, h) * cr;
+        }
+      if (interior(Nx, Ny, i, j))
+        E += (h * h) * (B * (1.0 - n3[a]) + K * (1.0 - n3[a] * n3[a]));
+    }
+  return E;
+}
+
+static double cm_site_energy_d(const double* n, int Nx, int Ny, int j, int i, double h,
+                               double kappa, double B, double K, const double* d) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *n1 = n, *n2 = n + P, *n3 = n + 2 * P;
+  static const int ks[4] = {1, -1, 2, -2};
+  size_t a = (size_t)j * Nx + i;
+  double e = 0.0;
+  for (int mu = 0; mu < 2; ++mu)
+    for (int q = 0; q < 4; ++q) {
+      int k = ks[q], ak = k < 0 ? -k : k;
+      int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+      size_t b = (size_t)j2 * Nx + i2;
+      double w = interior(Nx, Ny, i2, j2) ? 1.0 : 2.0;
+      double ck = (k > 0 ? 1.0 : -1.0) * cw(ak, h);
+      double dx1 = n1[a] - n1[b], dx2 = n2[a] - n2[b], dx3 = n3[a] - n3[b];
+      double ex = Jw[ak] / (4.0 * (h * h)) * (dx1 * dx1 + dx2 * dx2 + dx3 * dx3);
+      double cr = dot_cross(d + 3 * mu, n1[a], n2[a], n3[a], n1[b], n2[b], n3[b]);
+      e += w * (ex + kappa * ck * cr);
+    }
+  e += B * (1.0 - n3[a]) + K * (1.0 - n3[a] * n3[a]);
+  return e;
+}
+
+static void cm_site_gradient_d(const double* n, int Nx, int Ny, int j, int i, double h,
+                               double kappa, double B, double K, const double* d, double G[3]) {
+  const size_t P = (size_t)Nx * Ny;
+  const double *n1 = n, *n2 = n + P, *n3 = n + 2 * P;
+  size_t a = (size_t)j * Nx + i;
+  const double x[3] = {Dx(n1, Nx, j, i, h), Dx(n2, Nx, j, i, h), Dx(n3, Nx, j, i, h)};
+  const double y[3] = {Dy(n1, Nx, j, i, h), Dy(n2, Nx, j, i, h), Dy(n3, Nx, j, i, h)};
+  const double* dx = d;
+  const double* dy = d + 3;
+  /* (D_mu n) x d_mu */
+  const double c[3] = {(x[1] * dx[2] - x[2] * dx[1]) + (y[1] * dy[2] - y[2] * dy[1]),
+                       (x[2] * dx[0] - x[0] * dx[2]) + (y[2] * dy[0] - y[0] * dy[2]),
+                       (x[0] * dx[1] - x[1] * dx[0]) + (y[0] * dy[1] - y[1] * dy[0])};
+  G[0] = -(Lx(n1, Nx, j, i, h) + Ly(n1, Nx, j, i, h)) + 2.0 * kappa * c[0];
+  G[1] = -(Lx(n2, Nx, j, i, h) + Ly(n2, Nx, j, i, h)) + 2.0 * kappa * c[1];
+  G[2] = -(Lx(n3, Nx, j, i, h) + Ly(n3, Nx, j, i, h)) + 2.0 * kappa * c[2] -
+         (B + 2.0 * K * n3[a]);
+}
+
 /* ------------------------------------------------------------ abelian Higgs */
 /* Functional (Table 2 with u = 1; BASELINE config 3):
  *   e = 1/2 |D phi|^2 + 1/2 (d1 A2 - d2 A1)^2 + (lambda/8)(1-|phi|^2)^2 ,  D = d - iA.
@@ -379,6 +456,8 @@ static void ah_site_gradient(const double* f, int Nx, int Ny, int j, int i, doub
 typedef struct {
   int theory, Nx, Ny;
   double h, kappa, B, K, lambda;
+  int dmi;       /* 0: kappa n.(curl n) (BASELINE, d_mu = -e_mu); 1: the table d below */
+  double d[6];   /* d_x, d_y of PAPER.md:196 eq. (5) */
 } orc_model;
 
 static int ncomp(int theory) { return theory == ORC_CM ? 3 : 4; }
@@ -400,7 +479,8 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
       q[a] = 0.0;
       if (!interior(Nx, Ny, i, j)) continue;
       if (m->theory == ORC_CM) {
-        e[a] = cm_site_energy(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K);
+        e[a] = m->dmi ? cm_site_energy_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d)
+                      : cm_site_energy(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K);
         q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h);
       } else {
         e[a] = which_energy ? ah_site_energy_literal(f, Nx, Ny, j, i, m->h, m->lambda)
@@ -423,7 +503,8 @@ void orc_gradient(const orc_model* m, const double* f, double* G) {
       double g[4] = {0, 0, 0, 0};
       if (interior(Nx, Ny, i, j)) {
         if (m->theory == ORC_CM)
-          cm_site_gradient(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, g);
+          if (m->dmi) cm_site_gradient_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d, g);
+          else cm_site_gradient(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, g);
         else
           ah_site_gradient(f, Nx, Ny, j, i, m->h, m->lambda, g);
       }

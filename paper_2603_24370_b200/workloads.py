@@ -20,6 +20,14 @@ SEED0 = 260324370
 CM, AH = 0, 1
 HALO = 2
 
+# DMI vectors (d_x, d_y) of PAPER.md:196 eq. (5), e_DMI = kappa sum_mu d_mu . (n x d_mu n)
+# (DESIGN R16).  BLOCH is BASELINE's kappa n.(curl n); NEEL its rotation by 90 degrees about e3 in
+# spin space (interfacial DMI); D2D its spin mirror y -> -y (the paper's dmi_term="Heusler",
+# PAPER.md:141, which selects the antiskyrmion sector).
+DMI_BLOCH = ((-1.0, 0.0, 0.0), (0.0, -1.0, 0.0))
+DMI_NEEL = ((0.0, -1.0, 0.0), (1.0, 0.0, 0.0))
+DMI_D2D = ((1.0, 0.0, 0.0), (0.0, -1.0, 0.0))
+
 
 @dataclass
 class Workload:
@@ -36,6 +44,7 @@ class Workload:
     batch: int = 1
     steps: int = 0
     B_batch: np.ndarray | None = None
+    dmi: tuple | None = None          # None = DMI_BLOCH through the library's default path
     fields: np.ndarray | None = field(default=None, repr=False)   # [batch][C][Ny][Nx] fp64
 
     @property
