@@ -83,6 +83,9 @@ typedef struct {
                            /* bit 1: one kernel per RK4 stage (the round-1 schedule, kept   */
                            /* for A/B measurements) instead of the two fused flow kernels   */
   int chunks_per_segment;  /* tuning: rows/4 each CTA of the flow kernels marches; 0 = auto */
+  const double* dmi_d;     /* chiral magnet, optional HOST array[6] = (d_x, d_y): the DMI term   */
+                           /* kappa sum_mu d_mu.(n x d_mu n) of PAPER.md:196 eq. (5) (DESIGN    */
+                           /* R16).  NULL = kappa n.(curl n), i.e. d_x = -e_x, d_y = -e_y       */
 } ss_params;
 
 /* Bytes of device workspace ss_create needs for this problem; 0 on invalid arguments. */

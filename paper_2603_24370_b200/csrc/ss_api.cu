@@ -119,6 +119,8 @@ struct ss_solver {
   int cur;  // which ping-pong buffer holds (phi, v)
   int cps[3];  // chunks per y-segment of flow kernels X, Y, V
   int integrator;
+  int ktheory;    // kernel family: kCM, kAH or kCMG (chiral magnet with a DMI table)
+  double dmi[6];  // (d_x, d_y) of the table
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
@@ -239,6 +241,8 @@ void* flow_func(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
   return flow_func_t<kCM, double>(kind);
 #endif
+  if (theory == kCMG)
+    return dtype == SS_F64 ? flow_func_t<kCMG, double>(kind) : flow_func_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? flow_func_t<kCM, double>(kind) : flow_func_t<kCM, float>(kind);
   return dtype == SS_F64 ? flow_func_t<kAH, double>(kind) : flow_func_t<kAH, float>(kind);
@@ -253,6 +257,8 @@ int flow_smem(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
   return flow_smem_t<kCM, double>(kind);
 #endif
+  if (theory == kCMG)
+    return dtype == SS_F64 ? flow_smem_t<kCMG, double>(kind) : flow_smem_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? flow_smem_t<kCM, double>(kind) : flow_smem_t<kCM, float>(kind);
   return dtype == SS_F64 ? flow_smem_t<kAH, double>(kind) : flow_smem_t<kAH, float>(kind);
@@ -268,6 +274,8 @@ int flow_threads(int theory, int dtype, int kind) {
 #ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
   return flow_threads_t<kCM, double>(kind);
 #endif
+  if (theory == kCMG)
+    return dtype == SS_F64 ? flow_threads_t<kCMG, double>(kind) : flow_threads_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
     return dtype == SS_F64 ? flow_threads_t<kCM, double>(kind) : flow_threads_t<kCM, float>(kind);
   return dtype == SS_F64 ? flow_threads_t<kAH, double>(kind) : flow_threads_t<kAH, float>(kind);
@@ -309,12 +317,13 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   a.jA = real((16.0 / 12.0) / (4.0 * h * h)); a.jB = real((-1.0 / 12.0) / (4.0 * h * h));
   a.hk = real(s->kappa / (12.0 * h));
   a.qs = real(1.0 / (4.0 * 3.14159265358979323846 * (12.0 * h) * (12.0 * h)));
+  for (int i = 0; i < 6; ++i) a.dk[i] = real(s->kappa / (12.0 * h) * s->dmi[i]);
   KernelNode n;
-  n.func = flow_func(s->theory, s->dtype, kind);
+  n.func = flow_func(s->ktheory, s->dtype, kind);
   const int NC = (s->Ny + FR - 1) / FR;
   n.grid = dim3(s->L.nseg, (NC + s->cps[kind] - 1) / s->cps[kind], s->batch);
-  n.block = dim3(flow_threads(s->theory, s->dtype, kind), 1, 1);
-  n.smem = (size_t)flow_smem(s->theory, s->dtype, kind);
+  n.block = dim3(flow_threads(s->ktheory, s->dtype, kind), 1, 1);
+  n.smem = (size_t)flow_smem(s->ktheory, s->dtype, kind);
   n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
   n.name = kind == KX   ? "flow_x_grad_energy_charge_stage2"
            : kind == KY ? "flow_y_stage34_combine_project_ke"
@@ -428,7 +437,10 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   *out = nullptr;
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
-  if (p->integrator == SS_VERLET && (p->flags & 2)) return SS_ERR_UNSUPPORTED;
+  if ((p->integrator == SS_VERLET || p->dmi_d) && (p->flags & 2)) return SS_ERR_UNSUPPORTED;
+  if (p->dmi_d)
+    for (int i = 0; i < 6; ++i)
+      if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;
   int ndev = 0;
   if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
     if (ndev == 0) snprintf(g_cuda_msg, sizeof(g_cuda_msg), "no CUDA device (libss has no CPU path)");
@@ -450,6 +462,11 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->log_cap = p->arrest_log_capacity > 0 ? p->arrest_log_capacity : 4096;
   s->flags = p->flags;
   s->integrator = p->integrator;
+  s->ktheory = theory;
+  if (theory == SS_THEORY_CHIRAL_MAGNET && p->dmi_d) {
+    s->ktheory = kCMG;
+    for (int i = 0; i < 6; ++i) s->dmi[i] = p->dmi_d[i];
+  }
   s->fields_set = false;
   s->cur = 0;
   s->steps_done = 0; s->launches = 0;
@@ -476,12 +493,12 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     for (int kind = 0; kind < 3; ++kind) {
-      void* f = flow_func(theory, p->dtype, kind);
-      const int smem = flow_smem(theory, p->dtype, kind);
+      void* f = flow_func(s->ktheory, p->dtype, kind);
+      const int smem = flow_smem(s->ktheory, p->dtype, kind);
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
       if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
       int o = 1;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, flow_threads(theory, p->dtype, kind), smem);
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, flow_threads(s->ktheory, p->dtype, kind), smem);
       if (!cuda_ok(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor") || o < 1) {
         delete s; return SS_ERR_CUDA;
       }

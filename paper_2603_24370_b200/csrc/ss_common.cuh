@@ -6,7 +6,7 @@
 
 namespace ss {
 
-constexpr int kCM = 0, kAH = 1;
+constexpr int kCM = 0, kAH = 1, kCMG = 2;  // kCMG: chiral magnet with a general DMI table
 constexpr int HALO = 2;  // PAPER.md:102 "fourth-order ... stencils and halo width two"
 
 // Row segment of the canonical reduction tree (DESIGN R10): per-row partial sums are stored
@@ -43,6 +43,8 @@ struct StageArgs {
   real kappa, K, lambda;
   real lap0, lap1, lap2;  // 60, 16, 1 / (12 h^2)
   real dm1, dm2, K2;      // 2 kappa (8, 1) / (12 h); 2 K
+  real jA, jB, hk, qs;    // J1/4h^2, J2/4h^2, kappa/(12h), 1/(4 pi (12h)^2)
+  real dk[6];             // kappa/(12h) * (d_x, d_y)   (general DMI table)
 };
 
 struct ReduceArgs {

@@ -55,6 +55,7 @@ struct FlowArgs {
   real lap0, lap1, lap2;          // 60, 16, 1 / (12 h^2)
   real dm1, dm2, K2;              // 2 kappa (8, 1) / (12 h); 2 K
   real jA, jB, hk, qs;            // J1/4h^2, J2/4h^2, kappa/(12h), 1/(4 pi (12h)^2)
+  real dk[6];                     // kappa/(12h) * (d_x, d_y)   (general DMI table)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {

@@ -184,6 +184,113 @@ struct CM {
   }
 };
 
+// ------------------------------------------- chiral magnet with a general DMI table
+// e_DMI = kappa sum_mu d_mu . (n x D_mu n)  (eq. (5); DESIGN R16); p.dk[0..2],
+// p.dk[3..5] = kappa/(12h) * (d_x, d_y).  Exchange, Zeeman, anisotropy, charge as in CM.
+template <typename real>
+struct CMG {
+  static constexpr int C = 3;
+
+  // weighted eq. (1) numerators of all three components: sum_k w_k (12h c_k) n(i + k mu)
+  template <typename Tile, typename W>
+  __device__ __forceinline__ static void numerators(const Tile& T, const W& w, real dx[3],
+                                                    real dy[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      dx[c] = real(8) * (real(w.wx(0)) * T(c, 0, 1) - real(w.wx(1)) * T(c, 0, -1)) -
+              (real(w.wx(2)) * T(c, 0, 2) - real(w.wx(3)) * T(c, 0, -2));
+      dy[c] = real(8) * (real(w.wy(0)) * T(c, 1, 0) - real(w.wy(1)) * T(c, -1, 0)) -
+              (real(w.wy(2)) * T(c, 2, 0) - real(w.wy(3)) * T(c, -2, 0));
+    }
+  }
+
+  // G = -(Lx+Ly) n + 2 kappa sum_mu (D_mu n) x d_mu - (B + 2K n3) e3 ;  a = -(G - (G.n) n)
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_from(const Tile& T, const P& p, real B,
+                                                    const real dx[3], const real dy[3], real a[3]) {
+    const real n[3] = {T(0, 0, 0), T(1, 0, 0), T(2, 0, 0)};
+    real G[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const real s1 = (T(c, 0, 1) + T(c, 0, -1)) + (T(c, 1, 0) + T(c, -1, 0));
+      const real s2 = (T(c, 0, 2) + T(c, 0, -2)) + (T(c, 2, 0) + T(c, -2, 0));
+      G[c] = p.lap2 * s2 + (p.lap0 * n[c] - p.lap1 * s1);
+    }
+    const real* kx = p.dk;
+    const real* ky = p.dk + 3;
+    G[0] += real(2) * ((dx[1] * kx[2] - dx[2] * kx[1]) + (dy[1] * ky[2] - dy[2] * ky[1]));
+    G[1] += real(2) * ((dx[2] * kx[0] - dx[0] * kx[2]) + (dy[2] * ky[0] - dy[0] * ky[2]));
+    G[2] += real(2) * ((dx[0] * kx[1] - dx[1] * kx[0]) + (dy[0] * ky[1] - dy[1] * ky[0]));
+    G[2] -= B + p.K2 * n[2];
+    const real gn = (G[0] * n[0] + G[1] * n[1]) + G[2] * n[2];
+    a[0] = gn * n[0] - G[0];
+    a[1] = gn * n[1] - G[1];
+    a[2] = gn * n[2] - G[2];
+  }
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real B, real a[3]) {
+    real dx[3], dy[3];
+    numerators(T, BulkW(), dx, dy);
+    accel_from(T, p, B, dx, dy, a);
+  }
+
+  // site-form energy and charge densities; wdx, wdy = the WEIGHTED numerators (halo rule R3)
+  template <typename Tile, typename P, typename W>
+  __device__ __forceinline__ static void densities_from(const Tile& T, const P& p, real B,
+                                                        const W& w, const real wdx[3],
+                                                        const real wdy[3], const real dx[3],
+                                                        const real dy[3], real& e, real& q) {
+    const real n[3] = {T(0, 0, 0), T(1, 0, 0), T(2, 0, 0)};
+    const int ks[4] = {1, -1, 2, -2};
+    real sA = real(0), sB = real(0);
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      real tx = real(0), ty = real(0);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const real ax = n[c] - T(c, 0, ks[s]), ay = n[c] - T(c, ks[s], 0);
+        tx += ax * ax;
+        ty += ay * ay;
+      }
+      const real t = real(w.wx(s)) * tx + real(w.wy(s)) * ty;
+      if (s < 2) sA += t; else sB += t;
+    }
+    const real* kx = p.dk;
+    const real* ky = p.dk + 3;
+    // kappa sum_mu d_mu . (n x D_mu n)
+    const real dmi =
+        (kx[0] * (n[1] * wdx[2] - n[2] * wdx[1]) + kx[1] * (n[2] * wdx[0] - n[0] * wdx[2]) +
+         kx[2] * (n[0] * wdx[1] - n[1] * wdx[0])) +
+        (ky[0] * (n[1] * wdy[2] - n[2] * wdy[1]) + ky[1] * (n[2] * wdy[0] - n[0] * wdy[2]) +
+         ky[2] * (n[0] * wdy[1] - n[1] * wdy[0]));
+    e = (p.jA * sA + p.jB * sB) + dmi + (B * (real(1) - n[2]) + p.K * (real(1) - n[2] * n[2]));
+    const real c1 = dx[1] * dy[2] - dx[2] * dy[1], c2 = dx[2] * dy[0] - dx[0] * dy[2],
+               c3 = dx[0] * dy[1] - dx[1] * dy[0];
+    q = p.qs * ((n[0] * c1 + n[1] * c2) + n[2] * c3);
+  }
+  template <typename Tile, typename P, typename W>
+  __device__ __forceinline__ static void densities(const Tile& T, const P& p, real B, const W& w,
+                                                   real& e, real& q) {
+    real dx[3], dy[3], wdx[3], wdy[3];
+    numerators(T, BulkW(), dx, dy);
+    numerators(T, w, wdx, wdy);
+    densities_from(T, p, B, w, wdx, wdy, dx, dy, e, q);
+  }
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real B,
+                                                              real a[3], real& e, real& q) {
+    real dx[3], dy[3];
+    numerators(T, BulkW(), dx, dy);
+    accel_from(T, p, B, dx, dy, a);
+    densities_from(T, p, B, BulkW(), dx, dy, dx, dy, e, q);
+  }
+
+  __device__ __forceinline__ static void project_field(real m[3]) { CM<real>::project_field(m); }
+  __device__ __forceinline__ static void project_velocity(real u[3], const real n[3]) {
+    CM<real>::project_velocity(u, n);
+  }
+};
+
 // ------------------------------------------------------------------ abelian Higgs
 template <typename real>
 struct AH {
@@ -323,5 +430,6 @@ struct AH {
 template <int THEORY, typename real> struct TheoryOf;
 template <typename real> struct TheoryOf<kCM, real> { using type = CM<real>; };
 template <typename real> struct TheoryOf<kAH, real> { using type = AH<real>; };
+template <typename real> struct TheoryOf<kCMG, real> { using type = CMG<real>; };
 
 }  // namespace ss

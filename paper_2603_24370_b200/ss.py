@@ -40,7 +40,7 @@ class ss_params(C.Structure):
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("stream", C.c_void_p), ("arrest_log_capacity", C.c_int64),
                 ("integrator", C.c_int), ("flags", C.c_int),
-                ("chunks_per_segment", C.c_int)]
+                ("chunks_per_segment", C.c_int), ("dmi_d", C.POINTER(C.c_double))]
 
 
 _dp = C.POINTER(C.c_double)
@@ -85,7 +85,8 @@ def _check(rc, where, allow=()):
     return rc
 
 
-def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, integrator=0):
+def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, integrator=0,
+            dmi=None):
     p = ss_params()
     p.dtype, p.batch, p.dt = int(dtype), int(batch), float(dt)
     p.kappa, p.B, p.K, p.lam = float(kappa), float(B), float(K), float(lam)
@@ -96,6 +97,11 @@ def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, 
     p.arrest_log_capacity = int(log_cap)
     p.integrator, p.flags = int(integrator), int(flags)
     p.chunks_per_segment = int(cps)
+    if dmi is not None:
+        flat = [float(x) for v in dmi for x in (v if hasattr(v, "__len__") else (v,))]
+        assert len(flat) == 6
+        keep = (keep, (C.c_double * 6)(*flat))
+        p.dmi_d = C.cast(keep[1], _dp)
     return p, keep
 
 
@@ -108,8 +114,8 @@ class Solver:
     """ss_create ... ss_destroy around torch-owned device memory and the current torch stream."""
 
     def __init__(self, theory, Nx, Ny, h, *, dtype=F64, batch=1, dt=0.0, kappa=0.0, B=0.0, K=0.0,
-                 lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, integrator=RK4, device="cuda:0",
-                 stream=None):
+                 lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, integrator=RK4, dmi=None,
+                 device="cuda:0", stream=None):
         self.theory, self.Nx, self.Ny, self.batch = int(theory), int(Nx), int(Ny), int(batch)
         self.C = 3 if theory == THEORY_CHIRAL_MAGNET else 4
         self.dtype = dtype
@@ -118,7 +124,7 @@ class Solver:
         self.device = torch.device(device)
         self._h = C.c_void_p()
         p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps,
-                          integrator)
+                          integrator, dmi)
         nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
         if nbytes == 0:
             raise SSError(ERR_ARG, "ss_workspace_bytes")
@@ -138,7 +144,7 @@ class Solver:
         return (self.batch, self.C, self.Ny, self.Nx)
 
     def close(self):
-        if getattr(self, "_h", None) and self._h.value:
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
             _lib.ss_destroy(self._h)
             self._h = C.c_void_p()
 
@@ -233,4 +239,4 @@ def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0,
     """Solver configured from a workloads.Workload (sizes and parameters only)."""
     return Solver(w.theory, w.Nx, w.Ny, w.h, dtype=dtype, batch=w.batch, dt=w.dt, kappa=w.kappa,
                   B=w.B, K=w.K, lam=w.lam, B_batch=w.B_batch, log_cap=log_cap, flags=flags,
-                  cps=cps, integrator=integrator, device=device)
+                  cps=cps, integrator=integrator, dmi=getattr(w, "dmi", None), device=device)

@@ -26,7 +26,8 @@ def _ss():
 
 def _model(w, b=0):
     B = w.B if w.B_batch is None else float(w.B_batch[b])
-    return oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam)
+    return oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam,
+                        dmi=w.dmi)
 
 
 def _floor(m, phi, E):
@@ -162,6 +163,22 @@ def test_verlet_fp32_and_graph_vs_direct():
     assert outs[0][2:] == outs[1][2:]
     with pytest.raises(ss.SSError):
         ss.solver_for(w, flags=ss.FLAG_STAGED, integrator=ss.VERLET)   # no staged Verlet
+
+
+@pytest.mark.parametrize("table", ["neel", "d2d", "random", "bloch"])
+def test_general_dmi_tables(table):
+    # PAPER.md:196 eq. (5) with a (d_x, d_y) table (DESIGN R16): Neel and D2d ("Heusler", with the
+    # mirrored = antiskyrmion ansatz), a random table, and the Bloch table through
+    # the general kernels; ragged lattice, both integrators
+    rng = np.random.default_rng(5)
+    dmi = {"neel": W.DMI_NEEL, "d2d": W.DMI_D2D, "bloch": W.DMI_BLOCH,
+           "random": tuple(map(tuple, rng.standard_normal((2, 3))))}[table]
+    w = W.cm_single(N=90, K=0.2, mirror=(table == "d2d"))
+    w.dmi = dmi
+    s, flows = _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50))
+    if table == "d2d":
+        assert abs(s.charge()[0] - 1.0) < 5e-3           # antiskyrmion
+    _run_parity(w, checkpoints=(1, 5, 20), integrator="verlet")
 
 
 def test_graph_and_direct_launch_agree_bitwise():
