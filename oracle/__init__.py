@@ -213,3 +213,47 @@ class Flow:
         out = (C.c_int64 * max(n, 1))()
         lib().orc_flow_arrests(self._h, out, n)
         return [int(out[i]) for i in range(n)]
+
+
+# ---------------------------------------------------------------- headless visualisation (R17)
+# CPU restatement of the colour map of ss_render (DESIGN R17, own definition: the paper,
+# PAPER.md:158-160, gives no formula): observable over the interior, its extrema, then
+# t = (v - min) / (max - min) through a 5-stop piecewise-linear map, one IEEE fp64 operation at a
+# time in this order, bytes by floor(x + 0.5); halo sites are 0.
+_STOPS = np.array([[0, 0, 128], [0, 128, 255], [255, 255, 255], [255, 128, 0], [128, 0, 0]],
+                  dtype=np.float64)
+
+
+def observable(m, f, which):
+    """which: 0 energy density e_i, 1 charge / flux density q_i, 2 order parameter (CM n3, AH |phi|);
+    [Ny][Nx] with NaN on the halo."""
+    f = _f64(f)
+    out = np.full((m.Ny, m.Nx), np.nan)
+    I = (slice(2, m.Ny - 2), slice(2, m.Nx - 2))
+    if which == 2:
+        v = f[2] if m.theory == CM else np.sqrt(f[0] * f[0] + f[1] * f[1])
+    else:
+        _, _, de, dq = energy_charge(m, f, densities=True)
+        v = de if which == 0 else dq
+    out[I] = v[I]
+    return out
+
+
+def colormap(values):
+    """values [Ny][Nx] (NaN = halo) -> ([Ny][Nx][4] uint8 RGBA, (min, max))."""
+    ok = ~np.isnan(values)
+    mn, mx = float(values[ok].min()), float(values[ok].max())
+    span = mx - mn
+    v = np.where(ok, values, mn)
+    t = (v - mn) / span if span > 0.0 else np.full_like(v, 0.5)
+    t4 = t * 4.0
+    seg = np.minimum(t4.astype(np.int64), 3)
+    u = t4 - seg
+    img = np.zeros(values.shape + (4,), dtype=np.uint8)
+    for k in range(3):
+        c0, c1 = _STOPS[seg, k], _STOPS[seg + 1, k]
+        x = (c0 + (c1 - c0) * u) + 0.5
+        img[..., k] = np.floor(x).astype(np.int64).astype(np.uint8)
+    img[..., 3] = 255
+    img[~ok] = 0
+    return img, (mn, mx)

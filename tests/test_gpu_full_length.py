@@ -1,0 +1,72 @@
+"""BASELINE.json's acceptance run: every config over its FULL length on the GPU, final energy and
+charge within 1e-9 relative of the CPU oracle's full-length run, identical arrest indices over the
+first 100 steps.  The oracle values are stored under tests/golden/full_length_<key>.json by
+tests/golden/make_full_length.py (oracle only, hours of CPU time); a config whose file has not been
+generated is skipped.  Relative differences of E use the floor max(|E|, h^2 sum|e_i|)."""
+import json
+import os
+
+import pytest
+import torch
+
+from paper_2603_24370_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+CASES = {
+    "c1": lambda: W.baseline_config(1),
+    "c2": lambda: W.baseline_config(2),
+    "c3l1": lambda: W.baseline_config(3, lam=1.0),
+    "c3l2": lambda: W.baseline_config(3, lam=2.0),
+    "c4": lambda: W.baseline_config(4),
+    "c5": lambda: W.baseline_config(5),
+}
+
+
+def _gold(key):
+    path = os.path.join(GOLD, f"full_length_{key}.json")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated (tests/golden/make_full_length.py {key})")
+    return json.load(open(path))
+
+
+@pytest.mark.parametrize("key", sorted(CASES))
+def test_full_length_final_energy_and_charge(key):
+    from paper_2603_24370_b200 import ss
+    g = _gold(key)
+    w = CASES[key]()
+    assert (w.Nx, w.Ny, w.steps) == (g["Nx"], g["Ny"], g["runs"][0]["steps"])
+    s = ss.solver_for(w)
+    s.set_fields(torch.from_numpy(w.fields).to("cuda:0"))
+    E0, Q0 = s.energy(), s.charge()
+    s.step(w.steps)
+    E, Q = s.energy(), s.charge()
+    st = s.status()
+    assert st["steps"] == w.steps and not any(st["nonfinite"])
+    for r in g["runs"]:
+        b = r["lattice"]
+        floor = max(abs(r["E"]), r["abs_density_sum_h2"])
+        assert abs(E0[b] - r["E0"]) <= 1e-12 * max(abs(r["E0"]), floor)
+        assert abs(Q0[b] - r["Q0"]) <= 1e-12 * max(1.0, abs(r["Q0"]))
+        assert abs(E[b] - r["E"]) <= 1e-9 * floor, (key, b, E[b], r["E"])
+        assert abs(Q[b] - r["Q"]) <= 1e-9 * max(1.0, abs(r["Q"])), (key, b, Q[b], r["Q"])
+        got, _ = s.arrests(b)
+        assert [n for n in got if n <= 100] == [n for n in r["arrests_first"] if n <= 100]
+        assert E[b] < r["E0"]                                # the flow lowered the energy
+
+
+def test_full_length_fp32_config4_energy_within_1e4():
+    from paper_2603_24370_b200 import ss
+    g = _gold("c4")
+    w = W.baseline_config(4)
+    s = ss.solver_for(w, dtype=ss.F32)
+    s.set_fields(torch.from_numpy(w.fields).to("cuda:0", dtype=torch.float32))
+    r = g["runs"][0]
+    done = 0
+    for step, E_ref, Q_ref, _ in r["trace"]:                 # sampled every 250 steps
+        s.step(step - done)
+        done = step
+        floor = max(abs(E_ref), r["abs_density_sum_h2"])
+        assert abs(s.energy()[0] - E_ref) <= 1e-4 * floor, (step, s.energy()[0], E_ref)
+    assert abs(s.charge()[0] - r["Q"]) <= 1e-4 * max(1.0, abs(r["Q"]))
