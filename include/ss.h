@@ -130,6 +130,17 @@ int ss_status(ss_solver* s, int64_t* steps_done, int64_t* n_arrests, int* nonfin
  * energy.  Writes min(count, cap) entries to steps_host, the total to *count. */
 int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int64_t* count);
 
+/* Headless visualisation (DESIGN R17): writes the image
+ * of one observable of lattice `lattice` as [Ny][Nx] RGBA8 words (R in the low byte) into
+ * rgba_dev (DEVICE memory), mapped linearly between the observable's extrema over the interior,
+ * which a device-side reduction finds; halo sites are 0 (transparent).  minmax_host (HOST
+ * array[2], may be NULL) receives the extrema and makes the call synchronise the stream.
+ * There is no window or GL interop. */
+enum { SS_OBS_ENERGY = 0,   /* site-form energy density e_i                                   */
+       SS_OBS_CHARGE = 1,   /* CM: degree density; AH: flux density / 2 pi                     */
+       SS_OBS_ORDER = 2 };  /* CM: n3; AH: |phi| (order-parameter magnitude)                   */
+int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double* minmax_host);
+
 /* Number of kernel launches (graph nodes included) enqueued by this handle so far. */
 int64_t ss_launch_count(const ss_solver* s);
 

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "ss_flow.cuh"
+#include "ss_render.cuh"
 #include "ss_kernels.cuh"
 
 using namespace ss;
@@ -126,6 +127,7 @@ struct ss_solver {
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
   cudaGraphExec_t step_exec[2];
   std::vector<LatticeState> host_state;
+  std::vector<double> Bb_host;  // per-lattice Zeeman field (host copy)
 
   void* phi(int i) const { return ws + L.off_phi[i]; }
   void* vel(int i) const { return ws + L.off_vel[i]; }
@@ -475,6 +477,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
 
   std::vector<double> bb(s->batch, p->B);
   if (p->B_batch) bb.assign(p->B_batch, p->B_batch + s->batch);
+  s->Bb_host = bb;
   cudaError_t e = cudaMemcpyAsync(s->ws + L.off_bb, bb.data(), s->batch * sizeof(double),
                                   cudaMemcpyHostToDevice, s->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);  // bb is a local
@@ -728,6 +731,56 @@ int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_ker
   for (auto& e : ev) cudaEventDestroy(e);
   for (int i = 0; i < n; ++i) ms_host[i] = acc[i] / reps;
   return rc;
+}
+
+}  // extern "C" (templates below)
+
+template <int THEORY, typename real>
+static int render_t(ss_solver* s, int obs, int lattice, void* rgba_dev, double* minmax_host) {
+  const FlowArgs<real>& fa = *reinterpret_cast<const FlowArgs<real>*>(s->eval_nodes[0][0].args.data());
+  RenderArgs<real> r;
+  memset(&r, 0, sizeof(r));
+  const size_t sites = (size_t)s->Nx * s->Ny;
+  r.phi = (const real*)s->phi(s->cur) + (size_t)lattice * s->C * sites;
+  r.val = (double*)s->acc(2);                 // a3 of the staged schedule: free in this one
+  r.part = r.val + sites;
+  r.nblocks = (int)((sites + 255) / 256);
+  r.minmax = r.part + 2 * (size_t)r.nblocks;
+  r.rgba = (unsigned int*)rgba_dev;
+  r.Nx = s->Nx; r.Ny = s->Ny; r.obs = obs;
+  r.B = real(s->Bb_host[lattice]);
+  observable_kernel<THEORY, real><<<r.nblocks, 256, 0, s->stream>>>(fa, r);
+  minmax_kernel<real><<<1, 1024, 0, s->stream>>>(r);
+  colormap_kernel<real><<<r.nblocks, 256, 0, s->stream>>>(r);
+  s->launches += 3;
+  CK(cudaGetLastError());
+  if (minmax_host) {
+    CK(cudaMemcpyAsync(minmax_host, r.minmax, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  return SS_OK;
+}
+
+extern "C" {
+
+int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double* minmax_host) {
+  if (!s || !rgba_dev || lattice < 0 || lattice >= s->batch || observable < 0 || observable > 2)
+    return SS_ERR_ARG;
+  if (!s->fields_set) return SS_ERR_STATE;
+  if (s->flags & 2) return SS_ERR_UNSUPPORTED;
+  // scratch: [Ny*Nx] values + block extrema must fit in one field array (C*sizeof(real) >= 12)
+  const size_t sites = (size_t)s->Nx * s->Ny;
+  if ((sites + 2 * ((sites + 255) / 256) + 2) * sizeof(double) > s->L.field_bytes)
+    return SS_ERR_UNSUPPORTED;
+  const bool f64 = s->dtype == SS_F64;
+  switch (s->ktheory) {
+    case kCM: return f64 ? render_t<kCM, double>(s, observable, lattice, rgba_dev, minmax_host)
+                         : render_t<kCM, float>(s, observable, lattice, rgba_dev, minmax_host);
+    case kAH: return f64 ? render_t<kAH, double>(s, observable, lattice, rgba_dev, minmax_host)
+                         : render_t<kAH, float>(s, observable, lattice, rgba_dev, minmax_host);
+    default:  return f64 ? render_t<kCMG, double>(s, observable, lattice, rgba_dev, minmax_host)
+                         : render_t<kCMG, float>(s, observable, lattice, rgba_dev, minmax_host);
+  }
 }
 
 const char* ss_kernel_name(const ss_solver* s, int i) {

@@ -24,13 +24,14 @@ F64, F32 = 0, 1
 OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE = \
     0, -1, -2, -3, -4, -5, -6
 RK4, VERLET = 0, 1
+OBS_ENERGY, OBS_CHARGE, OBS_ORDER = 0, 1, 2
 FLAG_NO_GRAPH = 1
 FLAG_STAGED = 2
 
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
            "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",
            "ss_step", "ss_energy", "ss_charge", "ss_kinetic", "ss_status", "ss_arrests",
-           "ss_launch_count", "ss_strerror"]
+           "ss_launch_count", "ss_strerror", "ss_render"]
 
 
 class ss_params(C.Structure):
@@ -64,6 +65,7 @@ _lib.ss_status.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64
 _lib.ss_arrests.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.c_int64,
                             C.POINTER(C.c_int64)]
 _lib.ss_launch_count.argtypes = [C.c_void_p]
+_lib.ss_render.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, _dp]
 _lib.ss_launch_count.restype = C.c_int64
 _lib.ss_strerror.argtypes = [C.c_int]
 _lib.ss_strerror.restype = C.c_char_p
@@ -229,6 +231,15 @@ class Solver:
         cnt = C.c_int64()
         _check(_lib.ss_arrests(self._h, int(lattice), buf, cap, C.byref(cnt)), "ss_arrests")
         return [int(buf[i]) for i in range(min(cnt.value, cap))], cnt.value
+
+    def render(self, observable=OBS_ENERGY, lattice=0):
+        """(rgba [Ny][Nx] uint8x4 CUDA tensor, (min, max)) of one observable (headless)."""
+        img = torch.empty((self.Ny, self.Nx, 4), dtype=torch.uint8, device=self.device)
+        mm = (C.c_double * 2)()
+        with torch.cuda.stream(self.stream):
+            _check(_lib.ss_render(self._h, int(observable), int(lattice),
+                                  C.c_void_p(img.data_ptr()), mm), "ss_render")
+        return img, (mm[0], mm[1])
 
     def launch_count(self) -> int:
         return _lib.ss_launch_count(self._h)
