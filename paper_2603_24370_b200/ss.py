@@ -161,17 +161,32 @@ class Solver:
                              f"{self.shape}")
         return C.c_void_p(t.data_ptr())
 
+    def _after_current(self):
+        """the solver's stream waits for work already queued on torch's current stream"""
+        cur = torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+
+    def _before_current(self):
+        """torch's current stream waits for what the solver's stream has queued"""
+        cur = torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
     def set_fields(self, fields, vel=None):
+        self._after_current()               # the inputs may still be being produced there
         _check(_lib.ss_set_fields(self._h, self._dev(fields, "fields"), self._dev(vel, "vel")),
                "ss_set_fields")
 
     def get_fields(self, want_vel=True):
         f = torch.empty(self.shape, dtype=self.torch_dtype, device=self.device)
         v = torch.empty_like(f) if want_vel else None
+        self._after_current()               # f, v were allocated on torch's current stream
         with torch.cuda.stream(self.stream):
             _check(_lib.ss_get_fields(self._h, C.c_void_p(f.data_ptr()),
                                       C.c_void_p(v.data_ptr()) if want_vel else None),
                    "ss_get_fields")
+        self._before_current()              # the outputs are used on torch's current stream
         return (f, v) if want_vel else f
 
     def _host(self, t, name):
@@ -236,9 +251,11 @@ class Solver:
         """(rgba [Ny][Nx] uint8x4 CUDA tensor, (min, max)) of one observable (headless)."""
         img = torch.empty((self.Ny, self.Nx, 4), dtype=torch.uint8, device=self.device)
         mm = (C.c_double * 2)()
+        self._after_current()
         with torch.cuda.stream(self.stream):
             _check(_lib.ss_render(self._h, int(observable), int(lattice),
                                   C.c_void_p(img.data_ptr()), mm), "ss_render")
+        self._before_current()
         return img, (mm[0], mm[1])
 
     def launch_count(self) -> int:

@@ -36,7 +36,7 @@ def test_render_matches_cpu_restatement(case):
     if case == "ah":
         w = W.ah_vortices(N=150, h=0.1, lam=1.0, count=2, min_sep=2.0)
     else:
-        w = W.cm_multi(N=250, count=3, margin=12.0, min_sep=14.0)
+        w = W.cm_multi(N=252 if case == "cm_f32" else 250, count=3, margin=12.0, min_sep=14.0)
     f32 = case == "cm_f32"
     s = ss.solver_for(w, dtype=ss.F32 if f32 else ss.F64)
     s.set_fields(torch.from_numpy(w.fields).to("cuda:0", dtype=torch.float32 if f32 else torch.float64))
