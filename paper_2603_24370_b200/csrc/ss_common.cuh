@@ -67,7 +67,36 @@ __device__ __forceinline__ double warp_tree(double v) {
   return v;
 }
 
+// Two horizontally adjacent fp32 sites computed side by side with the packed fp32 instructions of
+// sm_100 (FFMA2 / FADD2 / FMUL2): the fp32 build of the flow kernels is issue-bound, and one
+// thread owning the pair (x, x+1) halves both the arithmetic and the shared-memory instructions.
+struct f2 {
+  float2 v;
+  f2() = default;
+  __device__ __forceinline__ f2(float a) : v(make_float2(a, a)) {}
+  __device__ __forceinline__ f2(double a) : v(make_float2(float(a), float(a))) {}
+  __device__ __forceinline__ f2(int a) : v(make_float2(float(a), float(a))) {}
+  __device__ __forceinline__ f2(float a, float b) : v(make_float2(a, b)) {}
+  __device__ __forceinline__ explicit f2(float2 t) : v(t) {}
+};
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { return f2(__fadd2_rn(a.v, b.v)); }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { return f2(__fmul2_rn(a.v, b.v)); }
+__device__ __forceinline__ f2 operator-(f2 a) { return f2(make_float2(-a.v.x, -a.v.y)); }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { return a + (-b); }
+__device__ __forceinline__ f2 operator*(float a, f2 b) { return f2(a) * b; }
+__device__ __forceinline__ f2 operator*(f2 a, float b) { return a * f2(b); }
+__device__ __forceinline__ f2 operator+(f2 a, float b) { return a + f2(b); }
+__device__ __forceinline__ f2 operator+(float a, f2 b) { return f2(a) + b; }
+__device__ __forceinline__ f2 operator-(f2 a, float b) { return a - f2(b); }
+__device__ __forceinline__ f2 operator-(float a, f2 b) { return f2(a) - b; }
+__device__ __forceinline__ f2& operator+=(f2& a, f2 b) { a = a + b; return a; }
+__device__ __forceinline__ f2& operator-=(f2& a, f2 b) { a = a - b; return a; }
+__device__ __forceinline__ f2& operator*=(f2& a, f2 b) { a = a * b; return a; }
+// fused multiply-add written as a * b + c contracts to FFMA2 only through the intrinsic
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return f2(__ffma2_rn(a.v, b.v, c.v)); }
+
 template <typename real> __device__ __forceinline__ real rsqrt_(real x);
+template <> __device__ __forceinline__ f2 rsqrt_<f2>(f2 x) { return f2(rsqrtf(x.v.x), rsqrtf(x.v.y)); }
 template <> __device__ __forceinline__ double rsqrt_<double>(double x) { return rsqrt(x); }
 template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return rsqrtf(x); }
 

@@ -109,6 +109,9 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 #ifndef SS_NST_Y
 #define SS_NST_Y 1    // one stage + 3 CTAs/SM beats two stages + 2 CTAs/SM for kernel Y
 #endif
+#ifndef SS_F32_VEC
+#define SS_F32_VEC 2  // fp32 chiral magnet: horizontally adjacent sites per thread (packed f2)
+#endif
 #ifndef SS_MINB_X
 #define SS_MINB_X 3   // CTAs per SM the register allocation aims at
 #endif
@@ -121,7 +124,10 @@ struct FlowCfg {
   static constexpr int C = TheoryOf<THEORY, real>::type::C;
   static constexpr int SPT = KIND == KY ? SS_SPT_Y : SS_SPT_X;
   static constexpr int ROWT = FR / SPT;                          // thread rows
-  static constexpr int THREADS = FW * ROWT;
+  // columns per thread: 2 (packed f2 arithmetic) for the fp32 chiral magnet, else 1
+  static constexpr int VEC = (sizeof(real) == 4 && THEORY != kAH) ? SS_F32_VEC : 1;
+  static constexpr int LX = FW / VEC;                            // threads per row
+  static constexpr int THREADS = LX * ROWT;
   static constexpr int RING = KIND == KY ? SS_RING_Y : SS_RING_X;
   static constexpr int NST = KIND == KY ? SS_NST_Y : SS_NST_X;
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
@@ -139,7 +145,8 @@ struct FlowCfg {
   static constexpr int SMEM = OFF_BAR + NST * 8;
   static constexpr int WANTB = KIND == KY ? SS_MINB_Y : SS_MINB_X;
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
-  static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTB ? FITB : WANTB);
+  static constexpr int WANTV = WANTB * VEC;                      // half the threads: twice the CTAs
+  static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTV ? FITB : WANTV);
   static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small for a single barrier");
   __device__ __forceinline__ static int ring_row(int gy) {       // gy >= -RING
     return (RING & (RING - 1)) == 0 ? (gy & (RING - 1)) : (int)((unsigned)(gy + RING) % RING);
@@ -157,13 +164,39 @@ __device__ __forceinline__ double warp_tree2(double a, double b, int lane) {
   return mine;
 }
 
+// the value a thread computes with: one site, or two side by side
+template <typename real, int VEC> struct VecOf { using type = real; };
+template <> struct VecOf<float, 2> { using type = f2; };
+template <typename V, typename real> __device__ __forceinline__ V vload(const real* q) { return V(*q); }
+template <> __device__ __forceinline__ f2 vload<f2, float>(const float* q) {
+  return f2(*reinterpret_cast<const float2*>(q));
+}
+template <typename real> __device__ __forceinline__ void vstore(real* q, real v) { *q = v; }
+__device__ __forceinline__ void vstore(float* q, f2 v) { *reinterpret_cast<float2*>(q) = v.v; }
+__device__ __forceinline__ double vsum(double v) { return v; }
+__device__ __forceinline__ double vsum(float v) { return double(v); }
+__device__ __forceinline__ double vsum(f2 v) { return double(v.v.x) + double(v.v.y); }  // tree level 1
+__device__ __forceinline__ float vlo(f2 v) { return v.v.x; }
+__device__ __forceinline__ float vhi(f2 v) { return v.v.y; }
+template <typename T> __device__ __forceinline__ T vlo(T v) { return v; }
+template <typename T> __device__ __forceinline__ T vhi(T v) { return v; }
+
+// halo weights of two side-by-side sites (DESIGN R3)
+struct EdgeW2 {
+  EdgeW a, b;
+  __device__ __forceinline__ EdgeW2(int gx, int gy, int Nx, int Ny) : a(gx, gy, Nx, Ny), b(gx + 1, gy, Nx, Ny) {}
+  __device__ __forceinline__ f2 wx(int s) const { return f2(float(a.x[s]), float(b.x[s])); }
+  __device__ __forceinline__ f2 wy(int s) const { return f2(float(a.y[s]), float(b.y[s])); }
+};
+
 template <int THEORY, typename real, int KIND>
 __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
                                   FlowCfg<THEORY, real, KIND>::MINB)
     flow_kernel(const __grid_constant__ FlowArgs<real> p) {
-  using Th = typename TheoryOf<THEORY, real>::type;
   using Cfg = FlowCfg<THEORY, real, KIND>;
-  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT, NST = Cfg::NST;
+  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT, NST = Cfg::NST, VEC = Cfg::VEC;
+  using vreal = typename VecOf<real, VEC>::type;
+  using Th = typename TheoryOf<THEORY, vreal>::type;
   constexpr int NQ = KIND == KX ? 2 : (KIND == KY ? 1 : 3);  // partial-sum quantities
   extern __shared__ __align__(128) unsigned char smem[];
   real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3   V: phi'
@@ -172,14 +205,14 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + Cfg::OFF_BAR);
 
   const int tid = threadIdx.x;
-  const int tx = tid & (FW - 1), r0 = (tid >> 6) * SPT, lane = tid & 31;  // rows r0 .. r0+SPT-1
+  const int tx = (tid % Cfg::LX) * VEC, r0 = (tid / Cfg::LX) * SPT, lane = tid & 31;  // columns tx..tx+VEC-1, rows r0..r0+SPT-1
   const int Nx = p.Nx, Ny = p.Ny;
   const int b = blockIdx.z, x0 = blockIdx.x * FW;
   const int NC = (Ny + FR - 1) / FR;
   const int cs = blockIdx.y * p.cps, ce = min(cs + p.cps, NC);  // stencil chunks [cs, ce)
   const int f0 = max(cs - 1, 0), f1 = min(ce, NC - 1);          // fill chunks [f0, f1]
   const bool vz = KIND != KX ? (p.state[b].v_is_zero != 0) : false;
-  const real Bz = real(p.Bb[b]);
+  const vreal Bz = vreal(real(p.Bb[b]));
 
   if (tid == 0) {
 #pragma unroll
@@ -205,34 +238,34 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 
   // pointwise RK4 data of the thread's sites, carried from their fill to their stencil (Y):
   // [0,C) = (phi + dt vh) + dt^2/6 (a1 + a2),  [C,2C) = vh + dt/6 (a1 + 2 a2)
-  real keep_new[SPT][2 * C], keep_old[SPT][2 * C];
+  vreal keep_new[SPT][2 * C], keep_old[SPT][2 * C];
 #pragma unroll
   for (int k = 0; k < SPT; ++k)
 #pragma unroll
-    for (int c = 0; c < 2 * C; ++c) keep_new[k][c] = keep_old[k][c] = real(0);
+    for (int c = 0; c < 2 * C; ++c) keep_new[k][c] = keep_old[k][c] = vreal(real(0));
 
   // raw site (row, lx) of chunk f -> the two stage fields in the rings
-  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, real* keep) {
+  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, vreal* keep) {
     constexpr int RW = Cfg::RAWW;
     const int gx = x0 - HALO + lx, gy = f * FR + row;
     const bool inter = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
     const int ro = row * RW + lx + (Cfg::XPAD - HALO);
     const real* rphi = reinterpret_cast<const real*>(st);
     const real* rvel = reinterpret_cast<const real*>(st + Cfg::ARRB);
-    real A[C], Bf[C];
+    vreal A[C], Bf[C];
 #pragma unroll
-    for (int c = 0; c < C; ++c) A[c] = Bf[c] = rphi[c * FR * RW + ro];
+    for (int c = 0; c < C; ++c) A[c] = Bf[c] = vload<vreal>(rphi + c * FR * RW + ro);
     if (inter) {  // halo sites of every stage field are the frozen halo
       if (KIND == KX) {
 #pragma unroll
-        for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * rvel[c * FR * RW + ro];
+        for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * vload<vreal>(rvel + c * FR * RW + ro);
         Th::project_field(Bf);
       } else if (KIND == KV) {
         const real* ra = reinterpret_cast<const real*>(st + 2 * Cfg::ARRB);
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-          const real vh = vz ? real(0) : rvel[c * FR * RW + ro];
-          const real w = vh + p.hdt * ra[c * FR * RW + ro];
+          const vreal vh = vz ? vreal(real(0)) : vload<vreal>(rvel + c * FR * RW + ro);
+          const vreal w = vh + p.hdt * vload<vreal>(ra + c * FR * RW + ro);
           A[c] = A[c] + p.dt * w;
           if (keep) keep[c] = w;
         }
@@ -242,16 +275,16 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
         const real* ra2 = reinterpret_cast<const real*>(st + 3 * Cfg::ARRB);
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-          const real ph = A[c];
-          const real a1 = ra1[c * FR * RW + ro];
-          const real vh = vz ? real(0) : rvel[c * FR * RW + ro];
-          const real a2 = vz ? a1 : ra2[c * FR * RW + ro];
+          const vreal ph = A[c];
+          const vreal a1 = vload<vreal>(ra1 + c * FR * RW + ro);
+          const vreal vh = vz ? vreal(real(0)) : vload<vreal>(rvel + c * FR * RW + ro);
+          const vreal a2 = vz ? a1 : vload<vreal>(ra2 + c * FR * RW + ro);
           A[c] = (ph + p.hdt * vh) + p.qdt2 * a1;
-          const real base = ph + p.dt * vh;
+          const vreal base = ph + p.dt * vh;
           Bf[c] = base + p.hdt2 * a2;
           if (keep) {
             keep[c] = base + p.sdt2 * (a1 + a2);
-            keep[C + c] = vh + p.sdt * (a1 + real(2) * a2);
+            keep[C + c] = vh + p.sdt * (a1 + vreal(real(2)) * a2);
           }
         }
         Th::project_field(A);
@@ -261,8 +294,8 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     const int wo = Cfg::ring_row(gy) * FWP + lx;
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      ringA[c * RP + wo] = A[c];
-      if (KIND != KV) ringB[c * RP + wo] = Bf[c];
+      vstore(ringA + c * RP + wo, A[c]);
+      if (KIND != KV) vstore(ringB + c * RP + wo, Bf[c]);
     }
   };
 
@@ -278,7 +311,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     }
   };
 
-  const int gx = x0 + tx;
+  const int gx = x0 + tx;  // first column of the thread (pairs never straddle the halo: Nx % 4 == 0)
   const bool xin = gx >= HALO && gx < Nx - HALO;
   const bool xedge = gx < 2 * HALO || gx >= Nx - 2 * HALO;
 
@@ -289,9 +322,9 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       mbar_wait(&full[k % NST], (uint32_t)((k / NST) & 1));
 #pragma unroll
       for (int k2 = 0; k2 < SPT; ++k2) fill_site(st, f, r0 + k2, tx + HALO, keep_new[k2]);
-      if (tid < 4 * FR) {
-        const int q = tid & 3;
-        fill_site(st, f, tid >> 2, q < 2 ? q : FW + q, nullptr);
+      if (tid < 4 * FR / VEC) {  // the x-halo columns 0, 1, FW+2, FW+3 of the chunk's rows
+        const int q = tid % (4 / VEC) * VEC;
+        fill_site(st, f, tid / (4 / VEC), q < 2 ? q : FW + q, nullptr);
       }
     }
     __syncthreads();
@@ -305,9 +338,24 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       int rw[SPT + 4];
 #pragma unroll
       for (int j = 0; j < SPT + 4; ++j) rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
+      // tile accessor: component c, ring row slot j, x offset dx of the thread's first column;
+      // with two columns per thread the odd offsets are recombined from the aligned pairs
+      auto tile = [&](const real* ring, const vreal (&colr)[C][SPT + 4], const int (&rwr)[SPT + 4],
+                      int c, int j, int dx) -> vreal {
+        if constexpr (VEC == 1) {
+          return dx == 0 ? colr[c][j] : vreal(ring[c * RP + rwr[j] + dx]);
+        } else {
+          auto pr = [&](int dxe) -> vreal {
+            return dxe == 0 ? colr[c][j] : vload<vreal>(ring + c * RP + rwr[j] + dxe);
+          };
+          if (dx == 0 || dx == 2 || dx == -2) return pr(dx);
+          if (dx == 1) return vreal(vhi(pr(0)), vlo(pr(2)));
+          return vreal(vhi(pr(-2)), vlo(pr(0)));
+        }
+      };
       double s0[SPT], s1[SPT], s2[SPT];
       bool act[SPT];
-      real aA[SPT][C];
+      vreal aA[SPT][C];
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         s0[k] = s1[k] = s2[k] = 0.0;
@@ -318,49 +366,48 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       real* o1 = p.out1 + o;
       // The SPT sites of a thread share their column: its SPT+4 ring values per component are
       // loaded once into registers; only the x-neighbours are read per site.
-      real col[C][SPT + 4];
+      vreal col[C][SPT + 4];
       // ---- ring A (X: phi -> a1, e, q    Y: phi3 -> a3)
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringA[c * RP + rw[j]];
+        for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringA + c * RP + rw[j]);
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         if (act[k]) {
           const int gy = gy0 + k;
-          auto TA = [&](int c, int dy, int dx) -> real {
-            return dx == 0 ? col[c][k + dy + 2] : ringA[c * RP + rw[k + dy + 2] + dx];
-          };
+          auto TA = [&](int c, int dy, int dx) -> vreal { return tile(ringA, col, rw, c, k + dy + 2, dx); };
           if (KIND == KX || KIND == KV) {
-            real e, q;
+            vreal e, q;
             if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
               Th::accel(TA, p, Bz, aA[k]);
-              Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
+              if constexpr (VEC == 2) Th::densities(TA, p, Bz, EdgeW2(gx, gy, Nx, Ny), e, q);
+              else Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
             } else {
               Th::accel_densities_bulk(TA, p, Bz, aA[k], e, q);
             }
-            s0[k] = double(e);
-            s1[k] = double(q);
+            s0[k] = vsum(e);
+            s1[k] = vsum(q);
             if (KIND == KX) {
 #pragma unroll
-              for (int c = 0; c < C; ++c) o0[c * p.plane + k * Nx] = aA[k][c];
+              for (int c = 0; c < C; ++c) vstore(o0 + c * p.plane + k * Nx, aA[k][c]);
             } else {  // second half kick, tangent projection, KE
-              real fn[C], u[C];
+              vreal fn[C], u[C];
 #pragma unroll
               for (int c = 0; c < C; ++c) {
                 fn[c] = col[c][k + 2];
                 u[c] = keep_old[k][c] + p.hdt * aA[k][c];
               }
               Th::project_velocity(u, fn);
-              real v2 = real(0);
+              vreal v2 = vreal(real(0));
 #pragma unroll
               for (int c = 0; c < C; ++c) {
-                o0[c * p.plane + k * Nx] = fn[c];
-                o1[c * p.plane + k * Nx] = u[c];
-                p.out2[o + c * p.plane + k * Nx] = aA[k][c];
+                vstore(o0 + c * p.plane + k * Nx, fn[c]);
+                vstore(o1 + c * p.plane + k * Nx, u[c]);
+                vstore(p.out2 + o + c * p.plane + k * Nx, aA[k][c]);
                 v2 += u[c] * u[c];
               }
-              s2[k] = 0.5 * double(v2);
+              s2[k] = 0.5 * vsum(v2);
             }
           } else {
             Th::accel(TA, p, Bz, aA[k]);
@@ -372,36 +419,34 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 #pragma unroll
         for (int c = 0; c < C; ++c)
 #pragma unroll
-          for (int j = 0; j < SPT + 4; ++j) col[c][j] = ringB[c * RP + rw[j]];
+          for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringB + c * RP + rw[j]);
       }
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         if (KIND != KV && act[k]) {
-          auto TB = [&](int c, int dy, int dx) -> real {
-            return dx == 0 ? col[c][k + dy + 2] : ringB[c * RP + rw[k + dy + 2] + dx];
-          };
-          real aB[C];
+          auto TB = [&](int c, int dy, int dx) -> vreal { return tile(ringB, col, rw, c, k + dy + 2, dx); };
+          vreal aB[C];
           Th::accel(TB, p, Bz, aB);
           if (KIND == KX) {
 #pragma unroll
-            for (int c = 0; c < C; ++c) o1[c * p.plane + k * Nx] = aB[c];
+            for (int c = 0; c < C; ++c) vstore(o1 + c * p.plane + k * Nx, aB[c]);
           } else {
-            real fn[C], u[C];
+            vreal fn[C], u[C];
 #pragma unroll
             for (int c = 0; c < C; ++c) {
               fn[c] = keep_old[k][c] + p.sdt2 * aA[k][c];
-              u[c] = keep_old[k][C + c] + p.sdt * (real(2) * aA[k][c] + aB[c]);
+              u[c] = keep_old[k][C + c] + p.sdt * (vreal(real(2)) * aA[k][c] + aB[c]);
             }
             Th::project_field(fn);
             Th::project_velocity(u, fn);
-            real v2 = real(0);
+            vreal v2 = vreal(real(0));
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-              o0[c * p.plane + k * Nx] = fn[c];
-              o1[c * p.plane + k * Nx] = u[c];
+              vstore(o0 + c * p.plane + k * Nx, fn[c]);
+              vstore(o1 + c * p.plane + k * Nx, u[c]);
               v2 += u[c] * u[c];
             }
-            s0[k] = 0.5 * double(v2);
+            s0[k] = 0.5 * vsum(v2);
           }
         }
       }
@@ -409,7 +454,9 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       // segment are added (low + high) by flush_partials after the next barrier
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
-        double* rr = red + (((f & 1) * 3) * FR + r0 + k) * 2 + (tx >> 5);
+        // VEC == 2: one warp holds the whole 64-site row segment (pair sums = tree level 1)
+        double* rr = red + (((f & 1) * 3) * FR + r0 + k) * 2 + (VEC == 2 ? 0 : (tx >> 5));
+        if (VEC == 2 && lane < NQ) rr[lane * FR * 2 + 1] = 0.0;
         if (KIND == KX || KIND == KV) {
           const double t = warp_tree2(s0[k], s1[k], lane);
           if (lane < 2) rr[lane * FR * 2] = t;

@@ -216,8 +216,8 @@ struct CMG {
       const real s2 = (T(c, 0, 2) + T(c, 0, -2)) + (T(c, 2, 0) + T(c, -2, 0));
       G[c] = p.lap2 * s2 + (p.lap0 * n[c] - p.lap1 * s1);
     }
-    const real* kx = p.dk;
-    const real* ky = p.dk + 3;
+    const auto* kx = p.dk;
+    const auto* ky = p.dk + 3;
     G[0] += real(2) * ((dx[1] * kx[2] - dx[2] * kx[1]) + (dy[1] * ky[2] - dy[2] * ky[1]));
     G[1] += real(2) * ((dx[2] * kx[0] - dx[0] * kx[2]) + (dy[2] * ky[0] - dy[0] * ky[2]));
     G[2] += real(2) * ((dx[0] * kx[1] - dx[1] * kx[0]) + (dy[0] * ky[1] - dy[1] * ky[0]));
@@ -255,8 +255,8 @@ struct CMG {
       const real t = real(w.wx(s)) * tx + real(w.wy(s)) * ty;
       if (s < 2) sA += t; else sB += t;
     }
-    const real* kx = p.dk;
-    const real* ky = p.dk + 3;
+    const auto* kx = p.dk;
+    const auto* ky = p.dk + 3;
     // kappa sum_mu d_mu . (n x D_mu n)
     const real dmi =
         (kx[0] * (n[1] * wdx[2] - n[2] * wdx[1]) + kx[1] * (n[2] * wdx[0] - n[0] * wdx[2]) +
