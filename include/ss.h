@@ -114,7 +114,8 @@ int ss_set_fields_host(ss_solver* s, const void* fields_host, const void* vel_ho
 int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
 
 /* Enqueue k flow steps (asynchronous; no host synchronisation, the arrest of eq. 4 is
- * decided on the device).  One step = RK4 stages 2-4 + update + projection, then the
+ * decided on the device; the steps are CUDA-graph replays, 8 steps per graph launch plus
+ * single-step graphs for the remainder).  One step = RK4 stages 2-4 + update + projection, then the
  * stencil pass on the new field (a, E, Q) and the arrest decision. */
 int ss_step(ss_solver* s, int64_t k);
 

@@ -33,6 +33,8 @@ inline bool cuda_ok(cudaError_t e, const char* what) {
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+constexpr int MULTI = 8;  // steps per multi-step graph (even)
+
 struct Layout {
   size_t field_bytes;  // one [batch][C][Ny][Nx] array
   size_t part_bytes;   // one [batch][Ny][nseg] fp64 array
@@ -125,7 +127,8 @@ struct ss_solver {
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
   std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
-  cudaGraphExec_t step_exec[2];
+  cudaGraphExec_t step_exec[2];   // one flow step, per ping-pong parity
+  cudaGraphExec_t multi_exec[2];  // MULTI consecutive steps in one graph (k steps per launch)
   std::vector<LatticeState> host_state;
   std::vector<double> Bb_host;  // per-lattice Zeeman field (host copy)
 
@@ -473,6 +476,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->cur = 0;
   s->steps_done = 0; s->launches = 0;
   s->step_exec[0] = s->step_exec[1] = nullptr;
+  s->multi_exec[0] = s->multi_exec[1] = nullptr;
   s->host_state.resize(s->batch);
 
   std::vector<double> bb(s->batch, p->B);
@@ -544,14 +548,27 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (rc != SS_OK) { ss_destroy(s); return rc; }
     }
   }
+  if (!(s->flags & 1)) {  // MULTI steps chained in one graph: fewer launches, no inter-graph gaps
+    for (int cur = 0; cur < 2; ++cur) {
+      std::vector<KernelNode> chain;
+      for (int i = 0; i < MULTI; ++i) {
+        const auto& one = s->step_nodes[(cur + i) & 1];
+        chain.insert(chain.end(), one.begin(), one.end());
+      }
+      int rc = build_graph(s, chain, &s->multi_exec[cur]);
+      if (rc != SS_OK) { ss_destroy(s); return rc; }
+    }
+  }
   *out = s;
   return SS_OK;
 }
 
 int ss_destroy(ss_solver* s) {
   if (!s) return SS_ERR_ARG;
-  for (int i = 0; i < 2; ++i)
+  for (int i = 0; i < 2; ++i) {
     if (s->step_exec[i]) cudaGraphExecDestroy(s->step_exec[i]);
+    if (s->multi_exec[i]) cudaGraphExecDestroy(s->multi_exec[i]);
+  }
   delete s;
   return SS_OK;
 }
@@ -637,6 +654,12 @@ int ss_step(ss_solver* s, int64_t k) {
     if (s->flags & 1) {
       int rc = launch_nodes(s, s->step_nodes[s->cur]);
       if (rc != SS_OK) return rc;
+    } else if (k - it >= MULTI) {  // MULTI is even: the parity is unchanged afterwards
+      CK(cudaGraphLaunch(s->multi_exec[s->cur], s->stream));
+      s->launches += (int64_t)MULTI * (int64_t)s->step_nodes[s->cur].size();
+      s->steps_done += MULTI;
+      it += MULTI - 1;
+      continue;
     } else {
       CK(cudaGraphLaunch(s->step_exec[s->cur], s->stream));
       s->launches += (int64_t)s->step_nodes[s->cur].size();
