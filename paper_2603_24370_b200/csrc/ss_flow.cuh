@@ -109,6 +109,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 #ifndef SS_NST_Y
 #define SS_NST_Y 1    // one stage + 3 CTAs/SM beats two stages + 2 CTAs/SM for kernel Y
 #endif
+#ifndef SS_BAR2_X
+#define SS_BAR2_X 0   // 1: a second barrier per chunk lets the ring shrink to 2*FR+2 rows
+#endif
+#ifndef SS_BAR2_Y
+#define SS_BAR2_Y 0
+#endif
 #ifndef SS_F32_VEC
 #define SS_F32_VEC 2  // fp32 chiral magnet: horizontally adjacent sites per thread (packed f2)
 #endif
@@ -147,7 +153,8 @@ struct FlowCfg {
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
   static constexpr int WANTV = WANTB * VEC;                      // half the threads: twice the CTAs
   static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTV ? FITB : WANTV);
-  static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small for a single barrier");
+  static constexpr bool BAR2 = KIND == KY ? SS_BAR2_Y : SS_BAR2_X;
+  static_assert(FR % SPT == 0 && RING >= (BAR2 ? 2 : 3) * FR + 2, "ring too small");
   __device__ __forceinline__ static int ring_row(int gy) {       // gy >= -RING
     return (RING & (RING - 1)) == 0 ? (gy & (RING - 1)) : (int)((unsigned)(gy + RING) % RING);
   }
@@ -474,6 +481,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     for (int k = 0; k < SPT; ++k)
 #pragma unroll
       for (int c = 0; c < 2 * C; ++c) keep_old[k][c] = keep_new[k][c];
+    if (Cfg::BAR2) __syncthreads();  // the next fill may overwrite rows this stencil read
   }
   __syncthreads();
   if (ce - 1 >= cs) flush_partials(ce - 1, ce & 1);
