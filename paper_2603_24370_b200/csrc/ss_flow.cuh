@@ -118,6 +118,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 #ifndef SS_F32_VEC
 #define SS_F32_VEC 2  // fp32 chiral magnet: horizontally adjacent sites per thread (packed f2)
 #endif
+#ifndef SS_SPT_F32
+#define SS_SPT_F32 1  // rows per thread of the packed fp32 kernels
+#endif
+#ifndef SS_MINB_F32
+#define SS_MINB_F32 5
+#endif
 #ifndef SS_MINB_X
 #define SS_MINB_X 3   // CTAs per SM the register allocation aims at
 #endif
@@ -128,10 +134,10 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 template <int THEORY, typename real, int KIND>
 struct FlowCfg {
   static constexpr int C = TheoryOf<THEORY, real>::type::C;
-  static constexpr int SPT = KIND == KY ? SS_SPT_Y : SS_SPT_X;
-  static constexpr int ROWT = FR / SPT;                          // thread rows
   // columns per thread: 2 (packed f2 arithmetic) for the fp32 chiral magnet, else 1
   static constexpr int VEC = (sizeof(real) == 4 && THEORY != kAH) ? SS_F32_VEC : 1;
+  static constexpr int SPT = VEC == 2 ? SS_SPT_F32 : (KIND == KY ? SS_SPT_Y : SS_SPT_X);
+  static constexpr int ROWT = FR / SPT;                          // thread rows
   static constexpr int LX = FW / VEC;                            // threads per row
   static constexpr int THREADS = LX * ROWT;
   static constexpr int RING = KIND == KY ? SS_RING_Y : SS_RING_X;
@@ -151,7 +157,7 @@ struct FlowCfg {
   static constexpr int SMEM = OFF_BAR + NST * 8;
   static constexpr int WANTB = KIND == KY ? SS_MINB_Y : SS_MINB_X;
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
-  static constexpr int WANTV = WANTB * VEC;                      // half the threads: twice the CTAs
+  static constexpr int WANTV = VEC == 2 ? SS_MINB_F32 : WANTB;
   static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTV ? FITB : WANTV);
   static constexpr bool BAR2 = KIND == KY ? SS_BAR2_Y : SS_BAR2_X;
   static_assert(FR % SPT == 0 && RING >= (BAR2 ? 2 : 3) * FR + 2, "ring too small");
