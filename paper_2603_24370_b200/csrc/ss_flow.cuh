@@ -13,16 +13,20 @@
 //       w = vh + dt/2 a, phi' = R(phi + dt w), a' = -Pi G(phi'), v' = Pi(w + dt/2 a')
 //
 // A CTA owns a strip of FW = 64 columns and a segment of rows, and marches down the segment in
-// chunks of FR = 4 rows; a thread owns SPT vertically adjacent sites of the chunk.  Per chunk f
-//   1. TMA (cp.async.bulk.tensor.3d, box {68, 4, C}, zero fill outside the lattice) has put the
-//      raw inputs of chunk f (+2 halo columns each side) into a 2-stage smem buffer;
-//   2. every thread turns its raw sites into the two stage fields and writes them into two
-//      smem rings of RING rows (the 16 x-halo sites are done by 16 threads);
-//   3. __syncthreads; thread 0 re-arms the stage with the TMA of chunk f+2;
-//   4. every thread evaluates both radius-2 stencils of its sites in chunk f-1 from the rings
-//      (rows f-1 +- 2 are there), stores the results with coalesced 64-wide row stores and
-//      contributes to the row-segment partial sums of the canonical tree.
-// No y-halo is ever re-read from HBM except one warm-up chunk per segment end.
+// chunks of FR = 4 rows; a thread owns SPT vertically adjacent sites of the chunk (fp32 chiral
+// magnet: VEC = 2 horizontally adjacent columns, computed with packed f2 arithmetic).  Per chunk f
+//   1. TMA (cp.async.bulk.tensor.3d, box {64 + 2 XPAD, 4, C}, zero fill outside the lattice, box
+//      start 16-byte aligned) has put the raw inputs of chunk f into an NST-stage smem buffer;
+//   2. every thread turns its raw sites into the stage field(s) and writes them into smem rings
+//      of RING rows x 68 columns (the 16 x-halo sites of the chunk are done by a few threads);
+//   3. __syncthreads; thread 0 re-arms the freed stage with the TMA of chunk f + NST;
+//   4. every thread evaluates the radius-2 stencil(s) of its sites in chunk f-1 from the rings
+//      (rows f-1 +- 2 are there; the sites of a thread share their column through registers),
+//      does the pointwise integrator algebra with data kept in registers since step 2, stores the
+//      results with coalesced row stores and contributes to the row-segment partial sums of the
+//      canonical tree (warp xor-shuffle tree, then low half + high half after the next barrier).
+// No y-halo is ever re-read from HBM except one warm-up chunk per segment end.  The switches
+// below (sites per thread, ring rows, TMA stages, CTAs per SM) were tuned on B200, DESIGN.md §6.
 #pragma once
 #include <cuda.h>
 
