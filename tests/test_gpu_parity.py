@@ -210,6 +210,37 @@ def test_fp32_energy_within_1e4_of_fp64_oracle():
     assert abs(s.charge()[0] - fl.charge) < 1e-4
 
 
+@pytest.mark.parametrize("case", ["cm", "cm_neel", "cm_verlet", "ah"])
+def test_fp32_fields_track_the_fp64_oracle_on_a_ragged_lattice(case):
+    # the packed two-column fp32 kernels (chiral magnet) and the scalar fp32 kernels (Abelian
+    # Higgs): fields after 12 steps within fp32 rounding of the fp64 oracle at EVERY site (edge
+    # rings with their halo weights included), energy and charge within 1e-4
+    ss = _ss()
+    if case == "ah":
+        w = W.ah_vortices(N=148, h=0.1, lam=1.0, count=2, min_sep=2.0)
+    else:
+        w = W.cm_multi(N=252, count=3, margin=12.0, min_sep=14.0)
+        w.K = 0.2
+        if case == "cm_neel":
+            w.dmi = W.DMI_NEEL
+    integ = "verlet" if case == "cm_verlet" else "rk4"
+    s = ss.solver_for(w, dtype=ss.F32, integrator=ss.VERLET if integ == "verlet" else ss.RK4)
+    s.set_fields(_dev(w.fields, torch.float32))
+    fl = oracle.Flow(_model(w), w.dt, integrator=integ)
+    fl.set_fields(w.fields[0])
+    E0 = s.energy()[0]
+    assert abs(E0 - fl.energy) <= 1e-5 * _floor(fl.m, w.fields[0], fl.energy)
+    s.step(12)
+    fl.step(12)
+    phi, vel = s.get_fields()
+    ophi, ovel = fl.get_fields()
+    assert np.abs(phi.cpu().numpy()[0] - ophi).max() <= 2e-5
+    assert np.abs(vel.cpu().numpy()[0] - ovel).max() <= 2e-4
+    assert abs(s.energy()[0] - fl.energy) <= 1e-4 * _floor(fl.m, ophi, fl.energy)
+    assert abs(s.charge()[0] - fl.charge) <= 1e-4 * max(1.0, abs(fl.charge))
+    assert abs(s.kinetic()[0] - fl.scalars()["KE"]) <= 1e-3 * max(fl.scalars()["KE"], 1e-6)
+
+
 def test_checkpoint_roundtrip_is_bit_exact():
     ss = _ss()
     w = W.cm_single(N=80)
