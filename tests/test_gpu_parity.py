@@ -241,6 +241,26 @@ def test_fp32_fields_track_the_fp64_oracle_on_a_ragged_lattice(case):
     assert abs(s.kinetic()[0] - fl.scalars()["KE"]) <= 1e-3 * max(fl.scalars()["KE"], 1e-6)
 
 
+@pytest.mark.timeout(120)
+def test_fp32_smallest_and_odd_multiple_lattices():
+    # smallest legal fp32 lattices (Nx % 4 == 0) and widths that are not a multiple of the strip
+    ss = _ss()
+    for Nx, Ny in ((8, 5), (8, 6), (12, 7), (68, 9), (132, 11)):
+        rng = np.random.default_rng(Nx * 10 + Ny)
+        f = rng.standard_normal((1, 3, Ny, Nx))
+        f /= np.sqrt((f * f).sum(1, keepdims=True))
+        w = W.Workload("tiny32", W.CM, Nx, Ny, 0.2, 0.1, kappa=1.0, B=0.6, K=0.1, fields=f)
+        for integ in ("rk4", "verlet"):
+            s = ss.solver_for(w, dtype=ss.F32, integrator=ss.VERLET if integ == "verlet" else ss.RK4)
+            s.set_fields(_dev(f, torch.float32))
+            fl = oracle.Flow(_model(w), w.dt, integrator=integ)
+            fl.set_fields(f[0])
+            s.step(5)
+            fl.step(5)
+            assert np.abs(s.get_fields()[0].cpu().numpy()[0] - fl.get_fields()[0]).max() <= 2e-5
+            assert abs(s.energy()[0] - fl.energy) <= 1e-4 * _floor(fl.m, fl.get_fields()[0], fl.energy)
+
+
 def test_checkpoint_roundtrip_is_bit_exact():
     ss = _ss()
     w = W.cm_single(N=80)
