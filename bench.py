@@ -272,7 +272,7 @@ def run_ours(args):
         raise RuntimeError("bench.py needs a CUDA device (libss has no CPU path)")
     dev = torch.device("cuda", local)
     torch.cuda.set_device(dev)
-    if world > 1:
+    if world > 1 and not dist.is_initialized():
         dist.init_process_group("nccl", device_id=dev)
 
     w, dtname = make_workload(args.workload)
@@ -392,14 +392,21 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
+    BAD = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
     r = run_ours(args)
+    remeasured = False
+    if BAD & set(r["clocks"]["reasons"]):       # thermal / hardware slowdown: re-measure once
+        time.sleep(10.0)
+        r["s"].close()
+        r = run_ours(args)
+        remeasured = True
     e2e = run_e2e(r, args)
     w = r["w"]
     cpu = None
     if r["rank"] == 0 and r["world"] == 1 and not args.no_cpu_baseline:
         cpu = time_oracle(w, args.cpu_seconds, integrator=args.integrator)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
-    bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"} & set(r["clocks"]["reasons"])
+    bad = BAD & set(r["clocks"]["reasons"])
     line = {
         "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": r["world"],
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms"] / args.steps,
@@ -414,7 +421,7 @@ def main():
                    if 7 * r["field_bytes"] > 3 * 126e6 else
                    "working set comparable to L2: not roofline evidence"},
         "e2e": e2e, "gpu_launches": r["launches"], "clocks": r["clocks"],
-        "clocks_rejected": sorted(bad),
+        "clocks_rejected": sorted(bad), "remeasured": remeasured,
         "roofline": r["roofline"], "cpu_baseline": cpu,
         "state": {"steps_done": r["status"]["steps"], "n_arrests": r["status"]["n_arrests"][:4]},
     }
