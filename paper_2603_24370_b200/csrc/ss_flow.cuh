@@ -128,6 +128,9 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
 #ifndef SS_MINB_F32
 #define SS_MINB_F32 5
 #endif
+#ifndef SS_AH_XY
+#define SS_AH_XY 1    // Abelian Higgs: DxDy A as D_y of per-row D_x values shared down the column
+#endif
 #ifndef SS_MINB_X
 #define SS_MINB_X 3   // CTAs per SM the register allocation aims at
 #endif
@@ -384,7 +387,26 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       // The SPT sites of a thread share their column: its SPT+4 ring values per component are
       // loaded once into registers; only the x-neighbours are read per site.
       vreal col[C][SPT + 4];
+      // Abelian Higgs: (12h)^2 DxDy A_c = D_y (D_x A_c) down the thread's column: one eq. (1)
+      // numerator per ring row (4 loads) shared by the SPT sites, instead of 16 loads per site
+      [[maybe_unused]] vreal xy[SPT][2];
+      [[maybe_unused]] auto mixed = [&](const real* ring) {
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+          vreal dxr[SPT + 4];
+#pragma unroll
+          for (int j = 0; j < SPT + 4; ++j) {
+            const real* q = ring + (2 + cc) * RP + rw[j];
+            dxr[j] = d1n<vreal>(vreal(q[-2]), vreal(q[-1]), vreal(q[1]), vreal(q[2]));
+          }
+#pragma unroll
+          for (int k = 0; k < SPT; ++k)
+            xy[k][cc] = d1n<vreal>(dxr[k], dxr[k + 1], dxr[k + 3], dxr[k + 4]);
+        }
+      };
+      constexpr bool AHXY = THEORY == kAH && VEC == 1 && SS_AH_XY;
       // ---- ring A (X: phi -> a1, e, q    Y: phi3 -> a3)
+      if constexpr (AHXY) mixed(ringA);
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
@@ -397,11 +419,13 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
           if (KIND == KX || KIND == KV) {
             vreal e, q;
             if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
-              Th::accel(TA, p, Bz, aA[k]);
+              if constexpr (AHXY) Th::accel_xy(TA, p, Bz, xy[k][0], xy[k][1], aA[k]);
+              else Th::accel(TA, p, Bz, aA[k]);
               if constexpr (VEC == 2) Th::densities(TA, p, Bz, EdgeW2(gx, gy, Nx, Ny), e, q);
               else Th::densities(TA, p, Bz, EdgeW(gx, gy, Nx, Ny), e, q);
             } else {
-              Th::accel_densities_bulk(TA, p, Bz, aA[k], e, q);
+              if constexpr (AHXY) Th::accel_densities_bulk_xy(TA, p, Bz, xy[k][0], xy[k][1], aA[k], e, q);
+              else Th::accel_densities_bulk(TA, p, Bz, aA[k], e, q);
             }
             s0[k] = vsum(e);
             s1[k] = vsum(q);
@@ -427,7 +451,8 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
               s2[k] = 0.5 * vsum(v2);
             }
           } else {
-            Th::accel(TA, p, Bz, aA[k]);
+            if constexpr (AHXY) Th::accel_xy(TA, p, Bz, xy[k][0], xy[k][1], aA[k]);
+            else Th::accel(TA, p, Bz, aA[k]);
           }
         }
       }
@@ -437,13 +462,15 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
         for (int c = 0; c < C; ++c)
 #pragma unroll
           for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringB + c * RP + rw[j]);
+        if constexpr (AHXY) mixed(ringB);
       }
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         if (KIND != KV && act[k]) {
           auto TB = [&](int c, int dy, int dx) -> vreal { return tile(ringB, col, rw, c, k + dy + 2, dx); };
           vreal aB[C];
-          Th::accel(TB, p, Bz, aB);
+          if constexpr (AHXY) Th::accel_xy(TB, p, Bz, xy[k][0], xy[k][1], aB);
+          else Th::accel(TB, p, Bz, aB);
           if (KIND == KX) {
 #pragma unroll
             for (int c = 0; c < C; ++c) vstore(o1 + c * p.plane + k * Nx, aB[c]);

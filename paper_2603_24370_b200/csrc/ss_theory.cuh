@@ -297,8 +297,14 @@ struct AH {
   static constexpr int C = 4;  // 0: Re phi, 1: Im phi, 2: A1, 3: A2
 
   template <typename Tile, typename P>
-  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real,
-                                               real a[4]) {
+  __device__ __forceinline__ static void accel(const Tile& T, const P& p, real B, real a[4]) {
+    accel_xy(T, p, B, Dxyn<real>(T, 2), Dxyn<real>(T, 3), a);
+  }
+  // xyA1, xyA2 = (12h)^2 DxDy A1, A2 at the site, supplied by the caller (the flow kernels form
+  // them as D_y of per-row D_x values shared by the vertically adjacent sites of a thread)
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_xy(const Tile& T, const P& p, real, real xyA1,
+                                                  real xyA2, real a[4]) {
     const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
     const real rho = p1 * p1 + p2 * p2, AA = A1 * A1 + A2 * A2;
     // S_mu,c = 12h * sum_k c_k (A_mu(i+k) + A_mu(i)) phi_c(i+k)
@@ -321,9 +327,9 @@ struct AH {
     const real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 + (Sx1 + Sy1) * p.i12h +
                     (AA - pot) * p2;
     const real ii = p.i12h * p.i12h;
-    const real G3 = -Lyn<real>(T, 2) * p.i12h2 + Dxyn<real>(T, 3) * ii +
+    const real G3 = -Lyn<real>(T, 2) * p.i12h2 + xyA2 * ii +
                     (p2 * Dxn<real>(T, 0) - p1 * Dxn<real>(T, 1)) * p.i12h + A1 * rho;
-    const real G4 = -Lxn<real>(T, 3) * p.i12h2 + Dxyn<real>(T, 2) * ii +
+    const real G4 = -Lxn<real>(T, 3) * p.i12h2 + xyA1 * ii +
                     (p2 * Dyn<real>(T, 0) - p1 * Dyn<real>(T, 1)) * p.i12h + A2 * rho;
     a[0] = -G1; a[1] = -G2; a[2] = -G3; a[3] = -G4;
   }
@@ -376,8 +382,14 @@ struct AH {
   // S_mu,c = sum_k c_k (A_mu,i + A_mu,j) phi_c,j of the force, and the mixed term is
   // 1/2 (A2 DxDy A1 + A1 DxDy A2) with the corner sums of the force.
   template <typename Tile, typename P>
-  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real,
+  __device__ __forceinline__ static void accel_densities_bulk(const Tile& T, const P& p, real B,
                                                               real a[4], real& e, real& q) {
+    accel_densities_bulk_xy(T, p, B, Dxyn<real>(T, 2), Dxyn<real>(T, 3), a, e, q);
+  }
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void accel_densities_bulk_xy(const Tile& T, const P& p, real,
+                                                                 real xyA1, real xyA2, real a[4],
+                                                                 real& e, real& q) {
     const real p1 = T(0, 0, 0), p2 = T(1, 0, 0), A1 = T(2, 0, 0), A2 = T(3, 0, 0);
     const real rho = p1 * p1 + p2 * p2, AA = A1 * A1 + A2 * A2;
     real Sx1, Sx2, Sy1, Sy2;
@@ -399,7 +411,6 @@ struct AH {
     const real G2 = -(Lxn<real>(T, 1) + Lyn<real>(T, 1)) * p.i12h2 + (Sx1 + Sy1) * p.i12h +
                     (AA - pot) * p2;
     const real ii = p.i12h * p.i12h;
-    const real xyA1 = Dxyn<real>(T, 2), xyA2 = Dxyn<real>(T, 3);
     const real dxA2 = Dxn<real>(T, 3), dyA1 = Dyn<real>(T, 2);
     const real G3 = -Lyn<real>(T, 2) * p.i12h2 + xyA2 * ii +
                     (p2 * Dxn<real>(T, 0) - p1 * Dxn<real>(T, 1)) * p.i12h + A1 * rho;
