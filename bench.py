@@ -233,14 +233,16 @@ KERNEL_UNITS = {
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-# captures (profiles/r01_ncu_full_{rk4,verlet}_cm4096_f64.csv, ..._rk4_cm4096_f32.csv); other
-# workloads: not captured.
+# captures (profiles/r01_ncu_full_{rk4,verlet}_cm4096_f64.csv, ..._rk4_cm4096_f32.csv,
+# ..._rk4_ah2048_f64.csv); other workloads: not captured.
 NCU_TRAFFIC = {
     ("cm_quench_4096", "f64", "flow_y_stage34_combine_project_ke"): 1.692745e9 + 779.828736e6,
     ("cm_quench_4096", "f64", "flow_x_grad_energy_charge_stage2"): 0.853236e9 + 768.891904e6,
     ("cm_quench_4096", "f64", "flow_v_verlet_step_energy_charge_ke"): 1.323498e9 + 1.169551e9,
     ("cm_quench_4096", "f32", "flow_y_stage34_combine_project_ke"): 843.659520e6 + 379.561216e6,
     ("cm_quench_4096", "f32", "flow_x_grad_energy_charge_stage2"): 428.198656e6 + 367.624960e6,
+    ("ah_vortices_2048_lam1", "f64", "flow_y_stage34_combine_project_ke"): 560.923136e6 + 237.878272e6,
+    ("ah_vortices_2048_lam1", "f64", "flow_x_grad_energy_charge_stage2"): 283.430144e6 + 224.302080e6,
 }
 
 
