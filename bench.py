@@ -55,12 +55,13 @@ def parse_args():
     ap.add_argument("--workload", default="cm4096_f64", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--staged", action="store_true", help="one kernel per RK4 stage (A/B)")
     ap.add_argument("--integrator", default="rk4", choices=["rk4", "verlet"],
                     help="rk4 = the metric's flow step (default); verlet = SURVEY 8(f) NEXT-1")
     ap.add_argument("--cps", type=int, default=0, help="chunks per segment (0 = auto)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0,
                     help="target CPU time of the oracle sample")
+    ap.add_argument("--sustained-seconds", type=float, default=2.5,
+                    help="length of the extra back-to-back run reported as `sustained` (0 = skip)")
     return ap.parse_args()
 
 
@@ -82,7 +83,7 @@ def peaks():
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML during the timed region."""
 
-    def __init__(self, index, period=0.02):
+    def __init__(self, index, period=0.002):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -123,8 +124,8 @@ class ClockSampler(threading.Thread):
         self._stop_evt.set()
         self.join(timeout=2.0)
         s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(s)}
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
 
 
 def nvml_index(torch, dev):
@@ -219,31 +220,48 @@ def run_reference(args):
 # Algorithmic bytes per interior site of each kernel of one flow step, in units of C*sizeof(real)
 # (DESIGN.md "Kernels and traffic model"): what the kernel must read + write once.
 KERNEL_UNITS = {
-    # two-kernel schedule (default)
     "flow_y_stage34_combine_project_ke": 6,   # reads phi, v, a1, a2 -> writes phi', v'
     "flow_x_grad_energy_charge_stage2": 4,    # reads phi', v'       -> writes a1, a2 (+ E, Q partials)
     # one-gradient-per-step integrator (--integrator verlet): reads phi, v, a -> phi', v', a'
     "flow_v_verlet_step_energy_charge_ke": 6,
-    # one kernel per RK4 stage (--staged, the first round-1 schedule)
-    "stage2": 3,                       # reads phi, v            -> writes a2
-    "stage3": 4,                       # reads phi, v, a1        -> writes a3
-    "stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
-    "stage1_grad_energy_charge": 2,    # reads phi'              -> writes a1 (+ E, Q partials)
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-# captures (profiles/r01_ncu_full_{rk4,verlet}_cm4096_f64.csv, ..._rk4_cm4096_f32.csv,
-# ..._rk4_ah2048_f64.csv); other workloads: not captured.
-NCU_TRAFFIC = {
-    ("cm_quench_4096", "f64", "flow_y_stage34_combine_project_ke"): 1.692745e9 + 779.828736e6,
-    ("cm_quench_4096", "f64", "flow_x_grad_energy_charge_stage2"): 0.853236e9 + 768.891904e6,
-    ("cm_quench_4096", "f64", "flow_v_verlet_step_energy_charge_ke"): 1.323498e9 + 1.169551e9,
-    ("cm_quench_4096", "f32", "flow_y_stage34_combine_project_ke"): 843.659520e6 + 379.561216e6,
-    ("cm_quench_4096", "f32", "flow_x_grad_energy_charge_stage2"): 428.198656e6 + 367.624960e6,
-    ("ah_vortices_2048_lam1", "f64", "flow_y_stage34_combine_project_ke"): 560.923136e6 + 237.878272e6,
-    ("ah_vortices_2048_lam1", "f64", "flow_x_grad_energy_charge_stage2"): 283.430144e6 + 224.302080e6,
-}
+# kernel name in bench.py -> the KIND template argument of flow_kernel<THEORY, real, KIND>
+KERNEL_KIND = {"flow_x_grad_energy_charge_stage2": 0, "flow_y_stage34_combine_project_ke": 1,
+               "flow_v_verlet_step_energy_charge_ke": 2}
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def ncu_traffic(workload_key, integrator, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, read from the newest
+    committed `ncu --set full` summary of this workload (profiles/rNN_ncu_full_<integrator>_
+    <workload>.csv: rows metric,unit,launch_0,...); None when no capture matches."""
+    import csv
+    import glob
+    import re
+    kind = KERNEL_KIND.get(kernel)
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles",
+                                          f"r*_ncu_full_{integrator}_{workload_key}.csv")))
+    for path in reversed(files):
+        try:
+            rows = {r[0]: r[1:] for r in csv.reader(open(path)) if r}
+            names = rows["Kernel Name"][1:]
+            col = None
+            for i, nm in enumerate(names):
+                m = re.search(r"flow_kernel<\s*\d+\s*,\s*\w+\s*,\s*(\d+)\s*>", nm)
+                if m and kind is not None and int(m.group(1)) == kind:
+                    col = i
+            if col is None:
+                continue
+            tot = 0.0
+            for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                unit, vals = rows[key][0], rows[key][1:]
+                tot += float(vals[col]) * _UNIT[unit]
+            return {"bytes": tot, "source": os.path.relpath(path, ROOT)}
+        except Exception:
+            continue
+    return None
 
 
 def max_over_ranks(values, dist=None, device="cpu"):
@@ -283,7 +301,6 @@ def run_ours(args):
     R = 8 if dtname == "f64" else 4
     host = torch.from_numpy(w.fields).to(tdt).contiguous().pin_memory()
     s = ss.solver_for(w, dtype=dtype, device=str(dev), cps=args.cps,
-                      flags=ss.FLAG_STAGED if args.staged else 0,
                       integrator=ss.VERLET if args.integrator == "verlet" else ss.RK4)
     s.set_fields(host.to(dev))
     sites = w.interior_sites
@@ -310,6 +327,25 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     ms = max_over_ranks([ms], dist if world > 1 else None, dev)[0]
     value = job_value(world, sites, args.steps, ms)
+
+    # ---- sustained: the same graph replays back to back for >= --sustained-seconds (the K-step
+    # region above can be a burst of a few tens of ms, before the power cap engages)
+    sustained = None
+    if args.sustained_seconds > 0:
+        n = int(min(400000, max(args.steps, args.sustained_seconds * 1e3 / (ms / args.steps))))
+        n = (n + 7) // 8 * 8
+        barrier()
+        sam2 = ClockSampler(nvml_index(torch, dev), period=0.01)
+        sam2.start()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(s.stream)
+        s.step(n)
+        f1.record(s.stream)
+        barrier()
+        c2 = sam2.stop()
+        ms2 = max_over_ranks([f0.elapsed_time(f1)], dist if world > 1 else None, dev)[0]
+        sustained = {"steps": n, "ms_per_step": ms2 / n, "seconds": ms2 * 1e-3,
+                     "value": job_value(world, sites, n, ms2), "unit": UNIT, "clocks": c2}
     st = s.status()
 
     # ---- per-kernel CUDA-event times of the same step (kernels launched one by one)
@@ -325,11 +361,21 @@ def run_ours(args):
             kern[name]["gbs"] = u * C * R * sites / (kms * 1e-3) / 1e9
     dom = max((n for n in kern if "gbs" in kern[n]), key=lambda n: kern[n]["ms"])
     tot = sum(k["ms"] for k in kern.values())
-    units = sum(KERNEL_UNITS.get(n, 0) for n in kern)      # 10 (two-kernel) or 16 (staged)
+    units = sum(KERNEL_UNITS.get(n, 0) for n in kern)      # 10 (RK4: Y + X) or 6 (Verlet)
+    for n in kern:
+        if "gbs" in kern[n]:
+            kern[n]["frac"] = kern[n]["gbs"] / peak
+            # which resource holds the kernel back: at >= 0.75 of the copy rate it is HBM itself,
+            # below that ncu shows dependency latency at 12 warps/SM
+            kern[n]["limiter"] = "hbm" if kern[n]["frac"] >= 0.75 else "latency (fp64 chains / smem, ncu)"
+            t = ncu_traffic(args.workload, args.integrator, n)
+            kern[n]["traffic"] = t["bytes"] if t else None
+    tr = ncu_traffic(args.workload, args.integrator, dom)
     roofline = {
-        "bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
+        "bound": "hbm", "limiter": kern[dom]["limiter"],
+        "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
         "unit": "GB/s", "frac": kern[dom]["gbs"] / peak,
-        "traffic": NCU_TRAFFIC.get((w.name, dtname, dom)),
+        "traffic": tr["bytes"] if tr else None, "traffic_source": tr["source"] if tr else None,
         "peak_source": peak_src, "kernel_ms": kern[dom]["ms"],
         "kernel_share_of_step": kern[dom]["ms"] / tot,
         "alg_bytes_per_site": KERNEL_UNITS[dom] * C * R,
@@ -346,6 +392,7 @@ def run_ours(args):
     }
     return dict(torch=torch, dist=dist, s=s, w=w, host=host, dev=dev, rank=rank, world=world,
                 value=value, ms=ms, launches=launches, clocks=clocks, roofline=roofline,
+                sustained=sustained,
                 status=st, sites=sites, field_bytes=field_bytes, dtname=dtname, barrier=barrier)
 
 
@@ -417,11 +464,12 @@ def main():
         "config": {"workload": w.name, "theory": "chiral_magnet" if w.theory == 0 else
                    "abelian_higgs", "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
                    "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
-                   "integrator": args.integrator, "schedule": "staged" if args.staged else "two-kernel",
+                   "integrator": args.integrator, "schedule": "two-kernel",
                    "parallelism": f"replicas x{r['world']}",
-                   "l2_policy": "working set (7 field arrays) larger than L2; no flush needed"
-                   if 7 * r["field_bytes"] > 3 * 126e6 else
+                   "l2_policy": "working set (6 field arrays) larger than L2; no flush needed"
+                   if 6 * r["field_bytes"] > 3 * 126e6 else
                    "working set comparable to L2: not roofline evidence"},
+        "sustained": r["sustained"],
         "e2e": e2e, "gpu_launches": r["launches"], "clocks": r["clocks"],
         "clocks_rejected": sorted(bad), "remeasured": remeasured,
         "roofline": r["roofline"], "cpu_baseline": cpu,

@@ -64,6 +64,10 @@ enum {
  * with the same projection (PAPER.md:129+154) and the same arrest (eq. 4). */
 enum { SS_RK4 = 0, SS_VERLET = 1 };
 
+/* ss_params.flags (debugging aid, not part of the method) */
+enum { SS_FLAG_NO_GRAPH = 1 }; /* launch the step's kernels one by one instead of replaying the
+                                  per-step CUDA graphs; results are bitwise identical */
+
 typedef struct {
   int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
                            /* reductions, E, Q, KE and the arrest test are always fp64      */
@@ -72,29 +76,40 @@ typedef struct {
   double kappa, B, K;      /* chiral magnet: DMI, Zeeman field, uniaxial anisotropy         */
   const double* B_batch;   /* optional HOST array[batch]: per-lattice B (overrides B)       */
   double lambda;           /* Abelian Higgs coupling (critical at 1)                        */
-  void* workspace;         /* DEVICE memory, >= ss_workspace_bytes, 256-byte aligned        */
+  void* workspace;         /* DEVICE memory, >= ss_workspace_bytes, 256-byte aligned; the   */
+                           /* solver runs on the device this memory lives on                */
   size_t workspace_bytes;
-  void* stream;            /* cudaStream_t owned by the caller; NULL = default stream       */
+  void* stream;            /* cudaStream_t of that device, owned by the caller; NULL =      */
+                           /* default stream                                                */
   int64_t arrest_log_capacity; /* entries per lattice; 0 -> 4096; later arrests are counted */
                                /* but not logged                                            */
   int integrator;          /* SS_RK4 | SS_VERLET                                            */
-  int flags;               /* bit 0: launch kernels one by one instead of replaying the     */
-                           /* per-step CUDA graph (debugging; same results)                 */
-                           /* bit 1: one kernel per RK4 stage (the round-1 schedule, kept   */
-                           /* for A/B measurements) instead of the two fused flow kernels   */
-  int chunks_per_segment;  /* tuning: rows/4 each CTA of the flow kernels marches; 0 = auto */
+  int flags;               /* 0 or SS_FLAG_NO_GRAPH                                         */
+  int chunks_per_segment;  /* tuning, 0 = auto: rows/4 each CTA of the flow kernels marches */
+                           /* (results do not depend on it)                                 */
   const double* dmi_d;     /* chiral magnet, optional HOST array[6] = (d_x, d_y): the DMI term   */
                            /* kappa sum_mu d_mu.(n x d_mu n) of PAPER.md:196 eq. (5) (DESIGN    */
                            /* R16).  NULL = kappa n.(curl n), i.e. d_x = -e_x, d_y = -e_y       */
 } ss_params;
 
-/* Bytes of device workspace ss_create needs for this problem; 0 on invalid arguments. */
+/* Limits of this build: 5 <= Nx <= 65536, 5 <= Ny <= 32768 (the device-side reduction tree of
+ * PAPER.md:158 / DESIGN R10 is finished by one warp per row and one CTA per lattice),
+ * 1 <= batch <= 65535; Nx even for SS_F64 and a multiple of 4 for SS_F32 (16-byte rows).
+ * Breaking an alignment or lower bound is SS_ERR_ARG, exceeding an upper bound is
+ * SS_ERR_UNSUPPORTED. */
+
+/* Bytes of device workspace ss_create needs for this problem (fields, velocities,
+ * accelerations of the Runge-Kutta stages, reduction buffers -- here two copies of phi and v, two
+ * acceleration arrays, partial sums, per-lattice state, arrest logs).  Returns 0 when ss_create
+ * would refuse the arguments (invalid or over a limit); p->workspace may be NULL here. */
 size_t ss_workspace_bytes(int theory, int Nx, int Ny, const ss_params* p);
 
 /* Create a solver (lattice, spacing, components and time step are fixed
- * before any device buffer is carved).  Requires Nx, Ny >= 5; Nx even for SS_F64 and a
- * multiple of 4 for SS_F32 (16-byte rows).  *out is NULL on failure. */
+ * before any device buffer is carved).  *out is NULL on failure.  The solver is bound to the
+ * device of p->workspace; every later call may be made with any device current. */
 int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_params* p);
+/* Release the handle (the device buffers are the caller's workspace and stream,
+ * which this call leaves untouched).  Pending work on the stream is not waited for. */
 int ss_destroy(ss_solver* s);
 
 /* Load fields (halo included, frozen from now on) and velocities (NULL = from rest,
@@ -120,40 +135,53 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
 int ss_step(ss_solver* s, int64_t k);
 
 /* Scalar read-outs: synchronise the stream, then fill HOST arrays of length batch.
- * Return SS_ERR_NONFINITE (after filling) if any lattice has a non-finite energy. */
-int ss_energy(ss_solver* s, double* E_host);  /* E_h of the current field                  */
-int ss_charge(ss_solver* s, double* Q_host);  /* CM: degree; AH: flux / 2 pi               */
-int ss_kinetic(ss_solver* s, double* KE_host); /* 1/2 h^2 sum |v|^2 of the last step,      */
-                                               /* before its arrest; 0 after ss_set_fields */
-/* steps_done: scalar; n_arrests, nonfinite: HOST arrays[batch]; any may be NULL. */
+ * Return SS_ERR_NONFINITE (after filling) if any lattice has a non-finite energy.
+ *   ss_energy   E_h[phi] of the current field: h^2 times the canonical-tree sum of the site-form
+ *               energy densities (PAPER.md:117 "discretized energy functional", :158 "total
+ *               energy ... parallel GPU reductions"; DESIGN R1, R3, R10).
+ *   ss_charge   topological charge ("conserved topological charge"; DESIGN R9):
+ *               CM degree (1/4 pi) h^2 sum n.(D_x n x D_y n), AH flux / 2 pi, same tree.
+ *   ss_kinetic  1/2 h^2 sum |v|^2 of the last step before its arrest ("kinetic
+ *               energy"; diagnostic, DESIGN R10); 0 after ss_set_fields. */
+int ss_energy(ss_solver* s, double* E_host);
+int ss_charge(ss_solver* s, double* Q_host);
+int ss_kinetic(ss_solver* s, double* KE_host);
+/* State of the arrest logic of PAPER.md:125-127 eq. (4).  steps_done: scalar; n_arrests,
+ * nonfinite: HOST arrays[batch]; any may be NULL.  Synchronises the stream. */
 int ss_status(ss_solver* s, int64_t* steps_done, int64_t* n_arrests, int* nonfinite);
-/* Arrest log of one lattice: the 1-based indices n+1 of the steps whose result raised the
- * energy.  Writes min(count, cap) entries to steps_host, the total to *count. */
+/* Arrest log of one lattice (eq. 4; DESIGN R8): the 1-based indices n+1 of
+ * the steps whose result raised the energy.  Writes min(count, cap, arrest_log_capacity)
+ * entries to steps_host (HOST), the total number of arrests to *count. */
 int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int64_t* count);
 
 /* Headless visualisation (DESIGN R17): writes the image
  * of one observable of lattice `lattice` as [Ny][Nx] RGBA8 words (R in the low byte) into
- * rgba_dev (DEVICE memory), mapped linearly between the observable's extrema over the interior,
- * which a device-side reduction finds; halo sites are 0 (transparent).  minmax_host (HOST
- * array[2], may be NULL) receives the extrema and makes the call synchronise the stream.
- * There is no window or GL interop. */
+ * rgba_dev (DEVICE memory), mapped linearly between the observable's extrema over the finite
+ * interior values, which a device-side reduction finds; halo sites are 0 (transparent), a
+ * non-finite interior value is opaque magenta.  minmax_host (HOST array[2], may be NULL)
+ * receives the extrema and makes the call synchronise the stream; only then can the call
+ * report SS_ERR_NONFINITE (image and extrema are still written).  No window, no GL interop. */
 enum { SS_OBS_ENERGY = 0,   /* site-form energy density e_i                                   */
        SS_OBS_CHARGE = 1,   /* CM: degree density; AH: flux density / 2 pi                     */
        SS_OBS_ORDER = 2 };  /* CM: n3; AH: |phi| (order-parameter magnitude)                   */
 int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double* minmax_host);
 
+const char* ss_strerror(int code);
+
+/* ---------------------------------------------------------------------------------------------
+ * Measurement-only entry points (used by bench.py and the tests; not part of the method).
+ * --------------------------------------------------------------------------------------------- */
+
 /* Number of kernel launches (graph nodes included) enqueued by this handle so far. */
 int64_t ss_launch_count(const ss_solver* s);
 
-/* Measurement aid: run `reps` real flow steps launching the step's kernels one by one with a
- * CUDA event between consecutive launches on the solver's stream, and return the average
- * device time of each kernel in milliseconds (HOST array, `cap` entries; *n_kernels = number
- * of kernels in one step, in launch order; ss_kernel_name(i) names entry i).  The state
- * advances by `reps` steps exactly as with ss_step(reps).  Synchronises the stream. */
+/* Run `reps` real flow steps launching the step's kernels one by one with a CUDA event between
+ * consecutive launches on the solver's stream, and return the average device time of each
+ * kernel in milliseconds (HOST array, `cap` entries; *n_kernels = number of kernels in one
+ * step, in launch order; ss_kernel_name(i) names entry i).  The state advances by `reps` steps
+ * exactly as with ss_step(reps).  Synchronises the stream. */
 int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_kernels);
 const char* ss_kernel_name(const ss_solver* s, int i);
-
-const char* ss_strerror(int code);
 
 #ifdef __cplusplus
 }

@@ -39,19 +39,27 @@ struct Layout {
   size_t field_bytes;  // one [batch][C][Ny][Nx] array
   size_t part_bytes;   // one [batch][Ny][nseg] fp64 array
   size_t rows_bytes;   // [batch][3][Ny]
-  size_t state_bytes, log_bytes, bb_bytes;
-  size_t off_phi[2], off_vel[2], off_a[3], off_part[3], off_rows, off_state, off_log, off_bb;
+  size_t state_bytes, log_bytes, bb_bytes, render_bytes;
+  size_t off_phi[2], off_vel[2], off_a[2], off_part[3], off_rows, off_state, off_log, off_bb;
+  size_t off_render;   // ss_render scratch: block extrema of one lattice, extrema, flag
   size_t total;
   int nseg;
 };
+
+// Limits of this build (include/ss.h "Limits"): the x-tree of row_reduce_kernel covers 32 lanes x
+// 32 segment partials of 64 sites, the y-tree of finalize_kernel 1024 threads x 32 rows, and the
+// lattice index is blockIdx.z.
+constexpr int MAX_NX = 65536, MAX_NY = 32768, MAX_BATCH = 65535;
+bool supported_shape(int Nx, int Ny, const ss_params* p) {
+  return Nx <= MAX_NX && Ny <= MAX_NY && p->batch <= MAX_BATCH;
+}
 
 bool valid_shape(int theory, int Nx, int Ny, const ss_params* p) {
   if (!p) return false;
   if (theory != SS_THEORY_CHIRAL_MAGNET && theory != SS_THEORY_ABELIAN_HIGGS) return false;
   if (p->dtype != SS_F64 && p->dtype != SS_F32) return false;
-  if (Nx < 5 || Ny < 5 || p->batch < 1 || p->batch > 65535) return false;  // grid.z
+  if (Nx < 5 || Ny < 5 || p->batch < 1) return false;
   if (p->dtype == SS_F64 ? (Nx % 2 != 0) : (Nx % 4 != 0)) return false;
-  if (Nx > 16384 || Ny > 32768) return false;  // reduction tree limits (32 lanes x 8, 1024 x 32)
   if (p->arrest_log_capacity < 0) return false;
   return true;
 }
@@ -68,15 +76,17 @@ Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
   L.state_bytes = align_up((size_t)p->batch * sizeof(LatticeState));
   L.log_bytes = align_up((size_t)p->batch * cap * sizeof(long long));
   L.bb_bytes = align_up((size_t)p->batch * sizeof(double));
+  L.render_bytes = align_up((2 * (((size_t)Nx * Ny + 255) / 256) + 4) * sizeof(double));
   size_t o = 0;
   for (int i = 0; i < 2; ++i) { L.off_phi[i] = o; o += L.field_bytes; }
   for (int i = 0; i < 2; ++i) { L.off_vel[i] = o; o += L.field_bytes; }
-  for (int i = 0; i < 3; ++i) { L.off_a[i] = o; o += L.field_bytes; }
+  for (int i = 0; i < 2; ++i) { L.off_a[i] = o; o += L.field_bytes; }
   for (int i = 0; i < 3; ++i) { L.off_part[i] = o; o += L.part_bytes; }
   L.off_rows = o; o += L.rows_bytes;
   L.off_state = o; o += L.state_bytes;
   L.off_log = o; o += L.log_bytes;
   L.off_bb = o; o += L.bb_bytes;
+  L.off_render = o; o += L.render_bytes;
   L.total = o;
   return L;
 }
@@ -89,28 +99,11 @@ struct KernelNode {
   const char* name;
 };
 
-template <int THEORY, typename real>
-void* stage_func(int stage) {
-  switch (stage) {
-    case 1: return (void*)stage_kernel<THEORY, real, 1>;
-    case 2: return (void*)stage_kernel<THEORY, real, 2>;
-    case 3: return (void*)stage_kernel<THEORY, real, 3>;
-    default: return (void*)stage_kernel<THEORY, real, 4>;
-  }
-}
-void* stage_func(int theory, int dtype, int stage) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return stage_func<kCM, double>(stage);
-#endif
-  if (theory == SS_THEORY_CHIRAL_MAGNET)
-    return dtype == SS_F64 ? stage_func<kCM, double>(stage) : stage_func<kCM, float>(stage);
-  return dtype == SS_F64 ? stage_func<kAH, double>(stage) : stage_func<kAH, float>(stage);
-}
-
 }  // namespace
 
 struct ss_solver {
   int theory, dtype, C, Nx, Ny, batch;
+  int device, sms;  // the device the workspace lives on (current at ss_create) and its SM count
   double h, dt, kappa, B, K, lambda;
   size_t R;
   cudaStream_t stream;
@@ -125,8 +118,8 @@ struct ss_solver {
   int ktheory;    // kernel family: kCM, kAH or kCMG (chiral magnet with a DMI table)
   double dmi[6];  // (d_x, d_y) of the table
   int64_t steps_done, launches;
-  std::vector<KernelNode> step_nodes[2];  // per parity: stages 2,3,4, stage 1, row_reduce, finalize
-  std::vector<KernelNode> eval_nodes[2];  // stage 1, row_reduce, finalize(advance = 0)
+  std::vector<KernelNode> step_nodes[2];  // per parity: Y, X (or V), row_reduce, finalize
+  std::vector<KernelNode> eval_nodes[2];  // X, row_reduce, finalize(advance = 0)
   cudaGraphExec_t step_exec[2];   // one flow step, per ping-pong parity
   cudaGraphExec_t multi_exec[2];  // MULTI consecutive steps in one graph (k steps per launch)
   std::vector<LatticeState> host_state;
@@ -141,62 +134,22 @@ struct ss_solver {
 
 namespace {
 
-template <typename real>
-KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return make_stage_node<double>(s, stage, cur);
-#endif
-  StageArgs<real> a;
-  memset(&a, 0, sizeof(a));
-  const double dt = s->dt, h = s->h;
-  a.phi = (const real*)s->phi(cur);
-  a.vel = (const real*)s->vel(cur);
-  a.aprev = stage == 3 ? (const real*)s->acc(0) : (const real*)s->acc(1);  // stage 4: a2
-  a.aout = (real*)s->acc(stage == 1 ? 0 : stage == 2 ? 1 : 2);
-  a.a1 = (const real*)s->acc(0);
-  a.a3 = (const real*)s->acc(2);
-  a.phi_out = (real*)s->phi(cur ^ 1);
-  a.vel_out = (real*)s->vel(cur ^ 1);
-  a.part_e = s->part(0);
-  a.part_q = s->part(1);
-  a.part_ke = s->part(2);
-  a.state = s->state();
-  a.Bb = (const double*)(s->ws + s->L.off_bb);
-  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg;
-  a.plane = (long long)s->Nx * s->Ny;
-  // stage fields (DESIGN "flow step"): phi2 = R(phi + dt/2 v), phi3 = R((phi + dt/2 v) + dt^2/4 a1),
-  // phi4 = R((phi + dt v) + dt^2/2 a2)
-  a.alpha = real(stage == 4 ? dt : 0.5 * dt);
-  a.beta = real(stage == 3 ? 0.25 * (dt * dt) : 0.5 * (dt * dt));
-  a.dt = real(dt);
-  a.sdt2 = real((dt * dt) / 6.0);
-  a.sdt = real(dt / 6.0);
-  a.i12h = real(1.0 / (12.0 * h));
-  a.i12h2 = real(1.0 / (12.0 * h * h));
-  a.kappa = real(s->kappa);
-  a.K = real(s->K);
-  a.lambda = real(s->lambda);
-  a.lap0 = real(60.0 / (12.0 * h * h)); a.lap1 = real(16.0 / (12.0 * h * h));
-  a.lap2 = real(1.0 / (12.0 * h * h));
-  a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
-  a.K2 = real(2.0 * s->K);
-  KernelNode n;
-  n.func = stage_func(s->theory, s->dtype, stage);
-  n.grid = dim3((s->Nx + TX - 1) / TX, (s->Ny + TY - 1) / TY, s->batch);
-  n.block = dim3(BX, BY, 1);
-  n.smem = (size_t)s->C * TYP * TXP * sizeof(real);
-  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
-  static const char* names[4] = {"stage1_grad_energy_charge", "stage2", "stage3",
-                                 "stage4_combine_project_ke"};
-  n.name = names[stage - 1];
-  return n;
-}
-
-KernelNode make_stage_node(const ss_solver* s, int stage, int cur) {
-  return s->dtype == SS_F64 ? make_stage_node<double>(s, stage, cur)
-                            : make_stage_node<float>(s, stage, cur);
-}
-
+// Every entry point runs on the solver's device whatever device is current in the calling thread
+// (the kernels, graph launches and copies carry no device of their own) and restores the caller's.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(const ss_solver* s) {
+    if (!s) return;
+    ok = cuda_ok(cudaGetDevice(&prev), "cudaGetDevice");
+    if (ok && prev != s->device) ok = cuda_ok(cudaSetDevice(s->device), "cudaSetDevice");
+    else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define GUARD(s)            \
+  DeviceGuard guard_(s);    \
+  if (!guard_.ok) return SS_ERR_CUDA
 
 // cuTensorMapEncodeTiled through the runtime (no link against libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
@@ -243,9 +196,6 @@ void* flow_func_t(int kind) {
                       : (void*)flow_kernel<THEORY, real, KV>;
 }
 void* flow_func(int theory, int dtype, int kind) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return flow_func_t<kCM, double>(kind);
-#endif
   if (theory == kCMG)
     return dtype == SS_F64 ? flow_func_t<kCMG, double>(kind) : flow_func_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
@@ -259,9 +209,6 @@ int flow_smem_t(int kind) {
                       : FlowCfg<THEORY, real, KV>::SMEM;
 }
 int flow_smem(int theory, int dtype, int kind) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return flow_smem_t<kCM, double>(kind);
-#endif
   if (theory == kCMG)
     return dtype == SS_F64 ? flow_smem_t<kCMG, double>(kind) : flow_smem_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
@@ -276,9 +223,6 @@ int flow_threads_t(int kind) {
                       : FlowCfg<THEORY, real, KV>::THREADS;
 }
 int flow_threads(int theory, int dtype, int kind) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return flow_threads_t<kCM, double>(kind);
-#endif
   if (theory == kCMG)
     return dtype == SS_F64 ? flow_threads_t<kCMG, double>(kind) : flow_threads_t<kCMG, float>(kind);
   if (theory == SS_THEORY_CHIRAL_MAGNET)
@@ -337,9 +281,6 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   return true;
 }
 bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
-#ifdef SS_FAST_BUILD  /* experiments: chiral magnet, fp64 only */
-  return make_flow_node<double>(s, kind, in, out);
-#endif
   return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out)
                             : make_flow_node<float>(s, kind, in, out);
 }
@@ -433,7 +374,7 @@ int read_state(ss_solver* s) {
 extern "C" {
 
 size_t ss_workspace_bytes(int theory, int Nx, int Ny, const ss_params* p) {
-  if (!valid_shape(theory, Nx, Ny, p)) return 0;
+  if (!valid_shape(theory, Nx, Ny, p) || !supported_shape(Nx, Ny, p)) return 0;
   return make_layout(theory, Nx, Ny, p).total;
 }
 
@@ -442,10 +383,11 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   *out = nullptr;
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
-  if ((p->integrator == SS_VERLET || p->dmi_d) && (p->flags & 2)) return SS_ERR_UNSUPPORTED;
+  if (p->flags & ~SS_FLAG_NO_GRAPH) return SS_ERR_ARG;
   if (p->dmi_d)
     for (int i = 0; i < 6; ++i)
       if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;
+  if (!supported_shape(Nx, Ny, p)) return SS_ERR_UNSUPPORTED;
   int ndev = 0;
   if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
     if (ndev == 0) snprintf(g_cuda_msg, sizeof(g_cuda_msg), "no CUDA device (libss has no CPU path)");
@@ -454,10 +396,15 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   Layout L = make_layout(theory, Nx, Ny, p);
   if (!p->workspace || p->workspace_bytes < L.total || ((uintptr_t)p->workspace & 255) != 0)
     return SS_ERR_WORKSPACE;
+  cudaPointerAttributes pa;
+  if (!cuda_ok(cudaPointerGetAttributes(&pa, p->workspace), "cudaPointerGetAttributes"))
+    return SS_ERR_CUDA;
+  if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return SS_ERR_WORKSPACE;
   ss_solver* s = new (std::nothrow) ss_solver();
   if (!s) return SS_ERR_ARG;
   s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_CHIRAL_MAGNET ? 3 : 4;
   s->Nx = Nx; s->Ny = Ny; s->batch = p->batch; s->h = h;
+  s->device = pa.device;
   s->dt = p->dt > 0.0 ? p->dt : 0.5 * h;
   s->kappa = p->kappa; s->B = p->B; s->K = p->K; s->lambda = p->lambda;
   s->R = p->dtype == SS_F64 ? 8 : 4;
@@ -478,51 +425,37 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->step_exec[0] = s->step_exec[1] = nullptr;
   s->multi_exec[0] = s->multi_exec[1] = nullptr;
   s->host_state.resize(s->batch);
+  DeviceGuard guard(s);
+  if (!guard.ok) { delete s; return SS_ERR_CUDA; }
+  s->sms = 0;
+  cudaError_t e = cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, s->device);
+  if (!cuda_ok(e, "cudaDeviceGetAttribute") || s->sms < 1) { delete s; return SS_ERR_CUDA; }
 
   std::vector<double> bb(s->batch, p->B);
   if (p->B_batch) bb.assign(p->B_batch, p->B_batch + s->batch);
   s->Bb_host = bb;
-  cudaError_t e = cudaMemcpyAsync(s->ws + L.off_bb, bb.data(), s->batch * sizeof(double),
-                                  cudaMemcpyHostToDevice, s->stream);
+  e = cudaMemcpyAsync(s->ws + L.off_bb, bb.data(), s->batch * sizeof(double),
+                      cudaMemcpyHostToDevice, s->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);  // bb is a local
   if (!cuda_ok(e, "upload B_batch")) { delete s; return SS_ERR_CUDA; }
 
-  const bool staged = (s->flags & 2) != 0;
-  if (staged) {
-    for (int stage = 1; stage <= 4; ++stage) {
-      void* f = stage_func(theory, p->dtype, stage);
-      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)((size_t)s->C * TYP * TXP * s->R));
-      if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+  for (int kind = 0; kind < 3; ++kind) {
+    void* f = flow_func(s->ktheory, p->dtype, kind);
+    const int smem = flow_smem(s->ktheory, p->dtype, kind);
+    e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+    int o = 1;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, flow_threads(s->ktheory, p->dtype, kind), smem);
+    if (!cuda_ok(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor") || o < 1) {
+      delete s; return SS_ERR_CUDA;
     }
-  } else {
-    int sms = 148, dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    for (int kind = 0; kind < 3; ++kind) {
-      void* f = flow_func(s->ktheory, p->dtype, kind);
-      const int smem = flow_smem(s->ktheory, p->dtype, kind);
-      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-      if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
-      int o = 1;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, f, flow_threads(s->ktheory, p->dtype, kind), smem);
-      if (!cuda_ok(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor") || o < 1) {
-        delete s; return SS_ERR_CUDA;
-      }
-      s->cps[kind] = p->chunks_per_segment > 0 ? p->chunks_per_segment
-                                               : choose_cps(L.nseg, Ny, s->batch, sms * o);
-    }
+    s->cps[kind] = p->chunks_per_segment > 0 ? p->chunks_per_segment
+                                             : choose_cps(L.nseg, Ny, s->batch, s->sms * o);
   }
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
-    if (staged) {
-      st.push_back(make_stage_node(s, 2, cur));
-      st.push_back(make_stage_node(s, 3, cur));
-      st.push_back(make_stage_node(s, 4, cur));
-      st.push_back(make_stage_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
-      ev.push_back(make_stage_node(s, 1, cur));
-    } else if (s->integrator == SS_VERLET) {
+    if (s->integrator == SS_VERLET) {
       KernelNode v, x0;
       if (!make_flow_node(s, KV, cur, &v) || !make_flow_node(s, KX, cur, &x0)) {
         ss_destroy(s);
@@ -543,12 +476,12 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     }
     make_reduce_nodes(s, 1, st);
     make_reduce_nodes(s, 0, ev);
-    if (!(s->flags & 1)) {
+    if (!(s->flags & SS_FLAG_NO_GRAPH)) {
       int rc = build_graph(s, st, &s->step_exec[cur]);
       if (rc != SS_OK) { ss_destroy(s); return rc; }
     }
   }
-  if (!(s->flags & 1)) {  // MULTI steps chained in one graph: fewer launches, no inter-graph gaps
+  if (!(s->flags & SS_FLAG_NO_GRAPH)) {  // MULTI steps chained in one graph: fewer launches, no inter-graph gaps
     for (int cur = 0; cur < 2; ++cur) {
       std::vector<KernelNode> chain;
       for (int i = 0; i < MULTI; ++i) {
@@ -565,22 +498,27 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
 
 int ss_destroy(ss_solver* s) {
   if (!s) return SS_ERR_ARG;
-  for (int i = 0; i < 2; ++i) {
-    if (s->step_exec[i]) cudaGraphExecDestroy(s->step_exec[i]);
-    if (s->multi_exec[i]) cudaGraphExecDestroy(s->multi_exec[i]);
+  {
+    DeviceGuard guard(s);
+    for (int i = 0; i < 2; ++i) {
+      if (s->step_exec[i]) cudaGraphExecDestroy(s->step_exec[i]);
+      if (s->multi_exec[i]) cudaGraphExecDestroy(s->multi_exec[i]);
+    }
   }
   delete s;
   return SS_OK;
 }
 
-// fields go to phi(0) and phi(1); velocities are staged in vel(1) (host source) or read from
-// the caller's array (device source) and masked to the interior into vel(0).
+// fields go to phi(0), their frozen halo also to phi(1) (a step writes only the interior of the
+// other ping-pong buffer); velocities are staged in vel(1) (host source) or read from the caller's
+// array (device source) and masked to the interior into vel(0); the halo of vel(1) is zeroed.
 static int set_fields_impl(ss_solver* s, const void* fields, const void* vel, cudaMemcpyKind kind) {
   if (!s || !fields) return SS_ERR_ARG;
+  GUARD(s);
   const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
   const long long planes = (long long)s->batch * s->C;
+  const int grid = s->sms * 8;
   CK(cudaMemcpyAsync(s->phi(0), fields, nbytes, kind, s->stream));
-  CK(cudaMemcpyAsync(s->phi(1), s->phi(0), nbytes, cudaMemcpyDeviceToDevice, s->stream));
   const void* vsrc = vel;
   if (vel && kind == cudaMemcpyHostToDevice) {
     CK(cudaMemcpyAsync(s->vel(1), vel, nbytes, kind, s->stream));
@@ -588,19 +526,25 @@ static int set_fields_impl(ss_solver* s, const void* fields, const void* vel, cu
   }
   if (vsrc) {
     if (s->dtype == SS_F64)
-      copy_interior_kernel<double><<<1184, 256, 0, s->stream>>>((double*)s->vel(0), (const double*)vsrc,
-                                                                 s->Nx, s->Ny, planes);
-    else
-      copy_interior_kernel<float><<<1184, 256, 0, s->stream>>>((float*)s->vel(0), (const float*)vsrc,
+      copy_interior_kernel<double><<<grid, 256, 0, s->stream>>>((double*)s->vel(0), (const double*)vsrc,
                                                                 s->Nx, s->Ny, planes);
+    else
+      copy_interior_kernel<float><<<grid, 256, 0, s->stream>>>((float*)s->vel(0), (const float*)vsrc,
+                                                               s->Nx, s->Ny, planes);
     s->launches += 1;
   } else {
     CK(cudaMemsetAsync(s->vel(0), 0, nbytes, s->stream));
   }
-  CK(cudaMemsetAsync(s->vel(1), 0, nbytes, s->stream));
+  if (s->dtype == SS_F64)
+    init_halo_kernel<double><<<grid, 256, 0, s->stream>>>((double*)s->phi(1), (double*)s->vel(1),
+                                                          (const double*)s->phi(0), s->Nx, s->Ny, planes);
+  else
+    init_halo_kernel<float><<<grid, 256, 0, s->stream>>>((float*)s->phi(1), (float*)s->vel(1),
+                                                         (const float*)s->phi(0), s->Nx, s->Ny, planes);
+  // KE partials are only written by a step: 0 after ss_set_fields
   for (int i = 0; i < 3; ++i) CK(cudaMemsetAsync(s->part(i), 0, s->L.part_bytes, s->stream));
   init_state_kernel<<<(s->batch + 127) / 128, 128, 0, s->stream>>>(s->state(), s->batch);
-  s->launches += 1;
+  s->launches += 2;
   CK(cudaGetLastError());
   s->cur = 0;
   s->steps_done = 0;
@@ -621,16 +565,18 @@ int ss_set_fields_host(ss_solver* s, const void* fields_host, const void* vel_ho
 static int get_fields_impl(ss_solver* s, void* fields, void* vel, cudaMemcpyKind kind) {
   if (!s) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   const size_t nbytes = (size_t)s->batch * s->C * s->Ny * s->Nx * s->R;
+  const int grid = s->sms * 8;
   if (fields) CK(cudaMemcpyAsync(fields, s->phi(s->cur), nbytes, kind, s->stream));
   if (vel) {
     const long long per = (long long)s->C * s->Ny * s->Nx;
     void* dst = kind == cudaMemcpyDeviceToHost ? s->vel(s->cur ^ 1) : vel;
     if (s->dtype == SS_F64)
-      export_velocity_kernel<double><<<1184, 256, 0, s->stream>>>(
+      export_velocity_kernel<double><<<grid, 256, 0, s->stream>>>(
           (double*)dst, (const double*)s->vel(s->cur), s->state(), per, s->batch);
     else
-      export_velocity_kernel<float><<<1184, 256, 0, s->stream>>>(
+      export_velocity_kernel<float><<<grid, 256, 0, s->stream>>>(
           (float*)dst, (const float*)s->vel(s->cur), s->state(), per, s->batch);
     s->launches += 1;
     CK(cudaGetLastError());
@@ -650,8 +596,9 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host) {
 int ss_step(ss_solver* s, int64_t k) {
   if (!s || k < 0) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   for (int64_t it = 0; it < k; ++it) {
-    if (s->flags & 1) {
+    if (s->flags & SS_FLAG_NO_GRAPH) {
       int rc = launch_nodes(s, s->step_nodes[s->cur]);
       if (rc != SS_OK) return rc;
     } else if (k - it >= MULTI) {  // MULTI is even: the parity is unchanged afterwards
@@ -673,6 +620,7 @@ int ss_step(ss_solver* s, int64_t k) {
 static int read_scalar(ss_solver* s, double* out, int which) {
   if (!s || !out) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   int rc = read_state(s);
   if (rc != SS_OK) return rc;
   bool bad = false;
@@ -690,6 +638,7 @@ int ss_kinetic(ss_solver* s, double* KE_host) { return read_scalar(s, KE_host, 2
 int ss_status(ss_solver* s, int64_t* steps_done, int64_t* n_arrests, int* nonfinite) {
   if (!s) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   int rc = read_state(s);
   if (rc != SS_OK) return rc;
   if (steps_done) *steps_done = s->steps_done;
@@ -706,6 +655,7 @@ int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int6
   if (!s || !count || lattice < 0 || lattice >= s->batch || cap < 0 || (cap > 0 && !steps_host))
     return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   int rc = read_state(s);
   if (rc != SS_OK) return rc;
   const int64_t total = s->host_state[lattice].n_arrests;
@@ -724,6 +674,7 @@ int ss_arrests(ss_solver* s, int lattice, int64_t* steps_host, int64_t cap, int6
 int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_kernels) {
   if (!s || !ms_host || !n_kernels || reps < 1) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
+  GUARD(s);
   const int n = (int)s->step_nodes[0].size();
   *n_kernels = n;
   if (cap < n) return SS_ERR_ARG;
@@ -765,21 +716,28 @@ static int render_t(ss_solver* s, int obs, int lattice, void* rgba_dev, double* 
   memset(&r, 0, sizeof(r));
   const size_t sites = (size_t)s->Nx * s->Ny;
   r.phi = (const real*)s->phi(s->cur) + (size_t)lattice * s->C * sites;
-  r.val = (double*)s->acc(2);                 // a3 of the staged schedule: free in this one
-  r.part = r.val + sites;
   r.nblocks = (int)((sites + 255) / 256);
+  r.part = (double*)(s->ws + s->L.off_render);
   r.minmax = r.part + 2 * (size_t)r.nblocks;
+  r.nonfinite = (int*)(r.minmax + 2);
   r.rgba = (unsigned int*)rgba_dev;
   r.Nx = s->Nx; r.Ny = s->Ny; r.obs = obs;
   r.B = real(s->Bb_host[lattice]);
+  CK(cudaMemsetAsync(r.nonfinite, 0, sizeof(int), s->stream));
   observable_kernel<THEORY, real><<<r.nblocks, 256, 0, s->stream>>>(fa, r);
   minmax_kernel<real><<<1, 1024, 0, s->stream>>>(r);
-  colormap_kernel<real><<<r.nblocks, 256, 0, s->stream>>>(r);
+  colormap_kernel<THEORY, real><<<r.nblocks, 256, 0, s->stream>>>(fa, r);
   s->launches += 3;
   CK(cudaGetLastError());
   if (minmax_host) {
-    CK(cudaMemcpyAsync(minmax_host, r.minmax, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    double out[3];  // min, max, flag word
+    CK(cudaMemcpyAsync(out, r.minmax, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
+    minmax_host[0] = out[0];
+    minmax_host[1] = out[1];
+    int flag;
+    memcpy(&flag, &out[2], sizeof(int));
+    if (flag) return SS_ERR_NONFINITE;
   }
   return SS_OK;
 }
@@ -790,11 +748,7 @@ int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double*
   if (!s || !rgba_dev || lattice < 0 || lattice >= s->batch || observable < 0 || observable > 2)
     return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
-  if (s->flags & 2) return SS_ERR_UNSUPPORTED;
-  // scratch: [Ny*Nx] values + block extrema must fit in one field array (C*sizeof(real) >= 12)
-  const size_t sites = (size_t)s->Nx * s->Ny;
-  if ((sites + 2 * ((sites + 255) / 256) + 2) * sizeof(double) > s->L.field_bytes)
-    return SS_ERR_UNSUPPORTED;
+  GUARD(s);
   const bool f64 = s->dtype == SS_F64;
   switch (s->ktheory) {
     case kCM: return f64 ? render_t<kCM, double>(s, observable, lattice, rgba_dev, minmax_host)

@@ -20,33 +20,6 @@ struct LatticeState {
   int v_is_zero, nonfinite;
 };
 
-template <typename real>
-struct StageArgs {
-  const real* phi;    // [batch][C][Ny][Nx] current field (halo frozen)
-  const real* vel;    // velocity
-  const real* aprev;  // acceleration entering the stage field (a1 for stage 3, a2 for stage 4)
-  real* aout;         // acceleration written by stages 1-3
-  const real* a1;     // stage 4 only
-  const real* a3;     // stage 4 only
-  real* phi_out;      // stage 4 only: phi^{n+1}
-  real* vel_out;      // stage 4 only: v^{n+1}
-  double* part_e;     // [batch][Ny][nseg] row-segment partial sums (stage 1)
-  double* part_q;
-  double* part_ke;    // (stage 4)
-  const LatticeState* state;
-  const double* Bb;   // [batch] Zeeman field per lattice
-  int Nx, Ny, nseg;
-  long long plane;    // Nx*Ny
-  real alpha, beta;   // stage field = R(phi + alpha*vhat + beta*aprev)
-  real dt, sdt2, sdt; // dt, dt^2/6, dt/6
-  real i12h, i12h2;   // 1/(12h), 1/(12h^2)
-  real kappa, K, lambda;
-  real lap0, lap1, lap2;  // 60, 16, 1 / (12 h^2)
-  real dm1, dm2, K2;      // 2 kappa (8, 1) / (12 h); 2 K
-  real jA, jB, hk, qs;    // J1/4h^2, J2/4h^2, kappa/(12h), 1/(4 pi (12h)^2)
-  real dk[6];             // kappa/(12h) * (d_x, d_y)   (general DMI table)
-};
-
 struct ReduceArgs {
   const double* part_e;  // [batch][Ny][nseg]
   const double* part_q;

@@ -25,8 +25,7 @@
 //      does the pointwise integrator algebra with data kept in registers since step 2, stores the
 //      results with coalesced row stores and contributes to the row-segment partial sums of the
 //      canonical tree (warp xor-shuffle tree, then low half + high half after the next barrier).
-// No y-halo is ever re-read from HBM except one warm-up chunk per segment end.  The switches
-// below (sites per thread, ring rows, TMA stages, CTAs per SM) were tuned on B200, DESIGN.md §6.
+// No y-halo is ever re-read from HBM except one warm-up chunk per segment end.
 #pragma once
 #include <cuda.h>
 
@@ -94,61 +93,25 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
       : "memory");
 }
 
-// tuning switches (defaults = the measured best); X = kernel X, Y = kernel Y
-#ifndef SS_SPT_X
-#define SS_SPT_X 2   // sites per thread
-#endif
-#ifndef SS_SPT_Y
-#define SS_SPT_Y 2
-#endif
-#ifndef SS_RING_X
-#define SS_RING_X 14  // ring rows: >= 14 (chunks f-1, f, f+1 and two rows of f-2 are live)
-#endif
-#ifndef SS_RING_Y
-#define SS_RING_Y 14
-#endif
-#ifndef SS_NST_X
-#define SS_NST_X 2    // TMA stages (chunks in flight while one is worked on)
-#endif
-#ifndef SS_NST_Y
-#define SS_NST_Y 1    // one stage + 3 CTAs/SM beats two stages + 2 CTAs/SM for kernel Y
-#endif
-#ifndef SS_BAR2_X
-#define SS_BAR2_X 0   // 1: a second barrier per chunk lets the ring shrink to 2*FR+2 rows
-#endif
-#ifndef SS_BAR2_Y
-#define SS_BAR2_Y 0
-#endif
-#ifndef SS_F32_VEC
-#define SS_F32_VEC 2  // fp32 chiral magnet: horizontally adjacent sites per thread (packed f2)
-#endif
-#ifndef SS_SPT_F32
-#define SS_SPT_F32 1  // rows per thread of the packed fp32 kernels
-#endif
-#ifndef SS_MINB_F32
-#define SS_MINB_F32 5
-#endif
-#ifndef SS_AH_XY
-#define SS_AH_XY 1    // Abelian Higgs: DxDy A as D_y of per-row D_x values shared down the column
-#endif
-#ifndef SS_MINB_X
-#define SS_MINB_X 3   // CTAs per SM the register allocation aims at
-#endif
-#ifndef SS_MINB_Y
-#define SS_MINB_Y 3
-#endif
+// Shape of the march, per kernel (measured on B200): 2 vertically adjacent
+// sites per thread, 14-row rings (chunks f-1, f, f+1 and two rows of f-2 are live, one barrier
+// per chunk), 3 CTAs per SM; two TMA stages in X and V, one in Y (so that the third CTA fits).
+// fp32 chiral magnet: 2 horizontally adjacent columns per thread (packed f2), 1 row, 5 CTAs/SM.
+constexpr int SPT_F64 = 2, SPT_F32V = 1;
+constexpr int RING_ROWS = 14;
+constexpr int MINB_F64 = 3, MINB_F32V = 5;
 
 template <int THEORY, typename real, int KIND>
 struct FlowCfg {
   static constexpr int C = TheoryOf<THEORY, real>::type::C;
   // columns per thread: 2 (packed f2 arithmetic) for the fp32 chiral magnet, else 1
-  static constexpr int VEC = (sizeof(real) == 4 && THEORY != kAH) ? SS_F32_VEC : 1;
-  static constexpr int SPT = VEC == 2 ? SS_SPT_F32 : (KIND == KY ? SS_SPT_Y : SS_SPT_X);
+  static constexpr int VEC = (sizeof(real) == 4 && THEORY != kAH) ? 2 : 1;
+  static constexpr int SPT = VEC == 2 ? SPT_F32V : SPT_F64;
   static constexpr int ROWT = FR / SPT;                          // thread rows
   static constexpr int LX = FW / VEC;                            // threads per row
   static constexpr int THREADS = LX * ROWT;
-  static constexpr int RING = KIND == KY ? SS_RING_Y : SS_RING_X;
-  static constexpr int NST = KIND == KY ? SS_NST_Y : SS_NST_X;
+  static constexpr int RING = RING_ROWS;
+  static constexpr int NST = KIND == KY ? 1 : 2;                 // TMA stages
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
   static constexpr int RAWW = FW + 2 * XPAD;                     // staged width (>= FWP)
   static constexpr int BOXB = C * FR * RAWW * (int)sizeof(real); // bytes one TMA box delivers
@@ -162,12 +125,10 @@ struct FlowCfg {
   static constexpr int OFF_RED = OFF_RING + NRING * RINGN * (int)sizeof(real);
   static constexpr int OFF_BAR = OFF_RED + 2 * 3 * FR * 2 * (int)sizeof(double);
   static constexpr int SMEM = OFF_BAR + NST * 8;
-  static constexpr int WANTB = KIND == KY ? SS_MINB_Y : SS_MINB_X;
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
-  static constexpr int WANTV = VEC == 2 ? SS_MINB_F32 : WANTB;
-  static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTV ? FITB : WANTV);
-  static constexpr bool BAR2 = KIND == KY ? SS_BAR2_Y : SS_BAR2_X;
-  static_assert(FR % SPT == 0 && RING >= (BAR2 ? 2 : 3) * FR + 2, "ring too small");
+  static constexpr int WANTB = VEC == 2 ? MINB_F32V : MINB_F64;
+  static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTB ? FITB : WANTB);
+  static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small");
   __device__ __forceinline__ static int ring_row(int gy) {       // gy >= -RING
     return (RING & (RING - 1)) == 0 ? (gy & (RING - 1)) : (int)((unsigned)(gy + RING) % RING);
   }
@@ -404,7 +365,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
             xy[k][cc] = d1n<vreal>(dxr[k], dxr[k + 1], dxr[k + 3], dxr[k + 4]);
         }
       };
-      constexpr bool AHXY = THEORY == kAH && VEC == 1 && SS_AH_XY;
+      constexpr bool AHXY = THEORY == kAH && VEC == 1;
       // ---- ring A (X: phi -> a1, e, q    Y: phi3 -> a3)
       if constexpr (AHXY) mixed(ringA);
 #pragma unroll
@@ -518,7 +479,6 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     for (int k = 0; k < SPT; ++k)
 #pragma unroll
       for (int c = 0; c < 2 * C; ++c) keep_old[k][c] = keep_new[k][c];
-    if (Cfg::BAR2) __syncthreads();  // the next fill may overwrite rows this stencil read
   }
   __syncthreads();
   if (ce - 1 >= cs) flush_partials(ce - 1, ce & 1);

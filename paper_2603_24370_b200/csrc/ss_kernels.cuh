@@ -1,147 +1,10 @@
-// Kernels of the flow step (one launch per RK4 stage + two small reduction kernels).
-//
-// stage_kernel<THEORY, real, STAGE>   ("derivative ... energy gradient ... Runge-
-//   Kutta stages" fused into one pass per stage):
-//     phase 1  stage field psi = R(phi + alpha*vhat + beta*aprev) on the tile plus a halo of 2,
-//              recomputed from phi, v, a_prev instead of being stored by the previous stage
-//              (16*C*sizeof(real) bytes per site-step instead of 21*C*sizeof(real)) -> smem
-//     phase 2  a = -Pi_psi G(psi) from smem (eq. 1, 2 stencils)
-//       STAGE 1: psi = phi; also energy / charge densities -> row-segment partial sums
-//       STAGE 4: + RK4 combine, projections (PAPER.md:129+154), KE partial sums, writes the
-//                new (phi, v) into the other ping-pong buffer
-// row_reduce_kernel / finalize_kernel: canonical tree (DESIGN R10) + arrest (eq. 4) on device.
+// Small kernels of the flow step: the two reduction kernels that finish the canonical tree
+// (DESIGN R10) and take the arrest decision (eq. 4) on the device, and the helpers of
+// ss_set_fields / ss_get_fields.  The stencil work is in ss_flow.cuh.
 #pragma once
 #include "ss_theory.cuh"
 
 namespace ss {
-
-constexpr int TX = SEG;  // tile width  = row segment of the reduction tree
-constexpr int TY = 16;   // tile height
-constexpr int BX = 64, BY = 4;
-constexpr int TXP = TX + 2 * HALO, TYP = TY + 2 * HALO;
-
-template <typename real, int C>
-struct SmemTile {
-  real v[C][TYP][TXP];
-};
-
-template <int THEORY, typename real, int STAGE>
-__global__ void __launch_bounds__(BX* BY) stage_kernel(const __grid_constant__ StageArgs<real> p) {
-  using Th = typename TheoryOf<THEORY, real>::type;
-  constexpr int C = Th::C;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  SmemTile<real, C>& sm = *reinterpret_cast<SmemTile<real, C>*>(smem_raw);
-  __shared__ double red[3][TY][BX / 32];
-
-  const int Nx = p.Nx, Ny = p.Ny;
-  const int b = blockIdx.z;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const long long lat = (long long)b * C * p.plane;
-  const real* __restrict__ phi = p.phi + lat;
-  const real* __restrict__ vel = p.vel + lat;
-  const real* __restrict__ aprev = p.aprev + lat;
-  const int tid = threadIdx.y * BX + threadIdx.x;
-  const bool vz = (STAGE > 1) ? (p.state[b].v_is_zero != 0) : true;
-
-  // ---- phase 1: stage field on tile + halo
-  for (int idx = tid; idx < TYP * TXP; idx += BX * BY) {
-    const int ly = idx / TXP, lx = idx - ly * TXP;
-    const int gx = x0 - HALO + lx, gy = y0 - HALO + ly;
-    real m[C];
-#pragma unroll
-    for (int c = 0; c < C; ++c) m[c] = real(0);
-    if (gx >= 0 && gx < Nx && gy >= 0 && gy < Ny) {
-      const long long o = (long long)gy * Nx + gx;
-#pragma unroll
-      for (int c = 0; c < C; ++c) m[c] = phi[c * p.plane + o];
-      const bool inter = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
-      if (STAGE > 1 && inter) {
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-          const real vh = vz ? real(0) : vel[c * p.plane + o];
-          m[c] = m[c] + p.alpha * vh;
-          if (STAGE > 2) m[c] = m[c] + p.beta * aprev[c * p.plane + o];
-        }
-        Th::project_field(m);
-      }
-    }
-#pragma unroll
-    for (int c = 0; c < C; ++c) sm.v[c][ly][lx] = m[c];
-  }
-  __syncthreads();
-
-  // ---- phase 2
-  const int gx = x0 + threadIdx.x;
-  const real Bz = real(p.Bb[b]);
-  const int warp_in_row = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#pragma unroll 1
-  for (int r = 0; r < TY / BY; ++r) {
-    const int ly = r * BY + threadIdx.y;
-    const int gy = y0 + ly;
-    const bool active = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
-    double s0 = 0.0, s1 = 0.0;
-    if (active) {
-      const int cx = threadIdx.x + HALO, cy = ly + HALO;
-      auto T = [&](int c, int dy, int dx) -> real { return sm.v[c][cy + dy][cx + dx]; };
-      real a[C];
-      Th::accel(T, p, Bz, a);
-      const long long o = (long long)gy * Nx + gx;
-      if (STAGE < 4) {
-#pragma unroll
-        for (int c = 0; c < C; ++c) p.aout[lat + c * p.plane + o] = a[c];
-      }
-      if (STAGE == 1) {
-        real e, q;
-        EdgeW w(gx, gy, Nx, Ny);
-        Th::densities(T, p, Bz, w, e, q);
-        s0 = double(e);
-        s1 = double(q);
-      }
-      if (STAGE == 4) {
-        real f[C], u[C];
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-          const long long oc = c * p.plane + o;
-          const real vh = vz ? real(0) : vel[oc];
-          const real A1 = p.a1[lat + oc], A2 = aprev[oc], A3 = p.a3[lat + oc];
-          f[c] = (phi[oc] + p.dt * vh) + p.sdt2 * ((A1 + A2) + A3);
-          u[c] = vh + p.sdt * ((A1 + real(2) * A2) + (real(2) * A3 + a[c]));
-        }
-        Th::project_field(f);
-        Th::project_velocity(u, f);
-        real v2 = real(0);
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-          p.phi_out[lat + c * p.plane + o] = f[c];
-          p.vel_out[lat + c * p.plane + o] = u[c];
-          v2 += u[c] * u[c];
-        }
-        s0 = 0.5 * double(v2);
-      }
-    }
-    if (STAGE == 1 || STAGE == 4) {
-      s0 = warp_tree(s0);
-      if (STAGE == 1) s1 = warp_tree(s1);
-      if (lane == 0) {
-        red[0][ly][warp_in_row] = s0;
-        if (STAGE == 1) red[1][ly][warp_in_row] = s1;
-      }
-    }
-  }
-  if (STAGE == 1 || STAGE == 4) {
-    __syncthreads();
-    if (tid < TY && y0 + tid < Ny) {
-      const long long po = ((long long)b * Ny + (y0 + tid)) * p.nseg + blockIdx.x;
-      static_assert(BX / 32 == 2, "row segment = two warps");
-      if (STAGE == 1) {
-        p.part_e[po] = red[0][tid][0] + red[0][tid][1];
-        p.part_q[po] = red[1][tid][0] + red[1][tid][1];
-      } else {
-        p.part_ke[po] = red[0][tid][0] + red[0][tid][1];
-      }
-    }
-  }
-}
 
 // In-thread aligned pairwise tree over m (power of two, <= 32) consecutive values.
 __device__ __forceinline__ double chunk_tree(const double* src, long long first, long long n, int m) {
@@ -222,6 +85,33 @@ __global__ void copy_interior_kernel(real* dst, const real* src, int Nx, int Ny,
     const int x = int(i % Nx), y = int((i / Nx) % Ny);
     const bool inter = x >= HALO && x < Nx - HALO && y >= HALO && y < Ny - HALO;
     dst[i] = inter ? src[i] : real(0);
+  }
+}
+
+// the second ping-pong buffers: frozen halo of phi copied from the first, halo of v zero (a step
+// writes their interior before anything reads it); 4 (Nx + Ny - 4) sites per plane
+template <typename real>
+__global__ void init_halo_kernel(real* phi1, real* vel1, const real* phi0, int Nx, int Ny,
+                                 long long planes) {
+  const long long ring = 2LL * HALO * Nx + 2LL * HALO * (Ny - 2 * HALO);
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < planes * ring;
+       i += (long long)gridDim.x * blockDim.x) {
+    const long long pl = i / ring;
+    long long r = i % ring;
+    int x, y;
+    if (r < 2LL * HALO * Nx) {  // rows 0, 1, Ny-2, Ny-1
+      const int k = int(r / Nx);
+      y = k < HALO ? k : Ny - 2 * HALO + k;
+      x = int(r % Nx);
+    } else {                    // columns 0, 1, Nx-2, Nx-1 of the other rows
+      r -= 2LL * HALO * Nx;
+      const int k = int(r % (2 * HALO));
+      y = HALO + int(r / (2 * HALO));
+      x = k < HALO ? k : Nx - 2 * HALO + k;
+    }
+    const long long o = (pl * Ny + y) * Nx + x;
+    phi1[o] = phi0[o];
+    vel1[o] = real(0);
   }
 }
 

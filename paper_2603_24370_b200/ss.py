@@ -26,7 +26,6 @@ OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE 
 RK4, VERLET = 0, 1
 OBS_ENERGY, OBS_CHARGE, OBS_ORDER = 0, 1, 2
 FLAG_NO_GRAPH = 1
-FLAG_STAGED = 2
 
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
            "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",
@@ -129,6 +128,9 @@ class Solver:
                           integrator, dmi)
         nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
         if nbytes == 0:
+            # invalid or over a limit: ss_create tells which (it checks before touching memory)
+            _check(_lib.ss_create(C.byref(self._h), self.theory, self.Nx, self.Ny, float(h),
+                                  C.byref(p)), "ss_create")
             raise SSError(ERR_ARG, "ss_workspace_bytes")
         if not torch.cuda.is_available():
             raise SSError(ERR_CUDA, "ss_create (no CUDA device; libss has no CPU path)")
@@ -137,9 +139,9 @@ class Solver:
         p.workspace = self.workspace.data_ptr()
         p.workspace_bytes = nbytes
         p.stream = self.stream.cuda_stream
-        with torch.cuda.device(self.device):
-            _check(_lib.ss_create(C.byref(self._h), self.theory, self.Nx, self.Ny, float(h),
-                                  C.byref(p)), "ss_create")
+        # the library binds the solver to the workspace's device; no call needs it to be current
+        _check(_lib.ss_create(C.byref(self._h), self.theory, self.Nx, self.Ny, float(h),
+                              C.byref(p)), "ss_create")
 
     @property
     def shape(self):
@@ -247,14 +249,16 @@ class Solver:
         _check(_lib.ss_arrests(self._h, int(lattice), buf, cap, C.byref(cnt)), "ss_arrests")
         return [int(buf[i]) for i in range(min(cnt.value, cap))], cnt.value
 
-    def render(self, observable=OBS_ENERGY, lattice=0):
-        """(rgba [Ny][Nx] uint8x4 CUDA tensor, (min, max)) of one observable (headless)."""
+    def render(self, observable=OBS_ENERGY, lattice=0, strict=True):
+        """(rgba [Ny][Nx] uint8x4 CUDA tensor, (min, max)) of one observable (headless).
+        strict=False tolerates non-finite interior values (drawn magenta)."""
         img = torch.empty((self.Ny, self.Nx, 4), dtype=torch.uint8, device=self.device)
         mm = (C.c_double * 2)()
         self._after_current()
         with torch.cuda.stream(self.stream):
             _check(_lib.ss_render(self._h, int(observable), int(lattice),
-                                  C.c_void_p(img.data_ptr()), mm), "ss_render")
+                                  C.c_void_p(img.data_ptr()), mm), "ss_render",
+                   allow=() if strict else (ERR_NONFINITE,))
         self._before_current()
         return img, (mm[0], mm[1])
 

@@ -52,9 +52,15 @@ def test_workspace_bytes_host_logic():
     assert ss.workspace_bytes(7, 64, 64) == 0                              # unknown theory
     assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 4, 64) == 0         # no interior
     assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 64, 64, batch=0) == 0
+    # limits of this build (include/ss.h "Limits")
+    assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 65538, 8) == 0
+    assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 8, 32770) == 0
+    assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 8, 8, batch=65536) == 0
+    assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 65536, 8) > 0
+    assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 8, 32768) > 0
     cm = ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 64, 64)
     ah = ss.workspace_bytes(ss.THEORY_ABELIAN_HIGGS, 64, 64)
-    assert cm >= 7 * 3 * 64 * 64 * 8 and ah > cm
+    assert cm >= 6 * 3 * 64 * 64 * 8 and ah > cm         # phi, v twice; a1, a2
     assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 64, 64, batch=3) > 2 * cm
     assert ss.workspace_bytes(ss.THEORY_CHIRAL_MAGNET, 64, 64, dtype=ss.F32) < cm
     # config 4 fp64 fits one B200 (180 GB) with room to spare

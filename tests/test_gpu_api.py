@@ -126,3 +126,21 @@ def test_velocity_input_halo_is_ignored_and_output_halo_is_zero():
     fl.set_fields(w.fields[0], vel[0])
     fl.step(5)
     assert np.abs(a.get_fields()[0].cpu().numpy()[0] - fl.get_fields()[0]).max() <= 1e-11
+
+
+def test_solver_on_a_non_current_device():
+    # the library binds a solver to the device of its workspace: calls work with any
+    # device current.  Needs two GPUs.
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    ss = _ss()
+    w = W.cm_single(N=64)
+    ref = ss.solver_for(w)
+    ref.set_fields(_dev(w.fields))
+    ref.step(10)
+    torch.cuda.set_device(0)
+    s = ss.solver_for(w, device="cuda:1")
+    s.set_fields(torch.from_numpy(w.fields).to("cuda:1"))
+    s.step(10)
+    assert torch.equal(s.get_fields()[0].cpu(), ref.get_fields()[0].cpu())
+    assert s.energy() == ref.energy()

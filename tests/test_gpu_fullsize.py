@@ -23,10 +23,11 @@ def _floor(m, phi, E):
     return max(abs(E), m.h * m.h * float(np.abs(de).sum()), 1e-300)
 
 
-def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4"):
+def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4", vel=None):
     ss = _ss()
     s = ss.solver_for(w, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
-    s.set_fields(torch.from_numpy(w.fields).to("cuda:0"))
+    s.set_fields(torch.from_numpy(w.fields).to("cuda:0"),
+                 None if vel is None else torch.from_numpy(vel).to("cuda:0"))
     s.step(steps)
     phi, vel = s.get_fields()
     E, Q, KE = s.energy(), s.charge(), s.kinetic()
@@ -36,7 +37,7 @@ def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4
         B = w.B if w.B_batch is None else float(w.B_batch[b])
         m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam)
         fl = oracle.Flow(m, w.dt, integrator=integrator)
-        fl.set_fields(w.fields[b])
+        fl.set_fields(w.fields[b], None if vel is None else vel[b])
         fl.step(steps)
         ophi, ovel = fl.get_fields()
         gp, gv = phi[b].cpu().numpy(), vel[b].cpu().numpy()
@@ -63,6 +64,18 @@ def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4
 
 def test_config4_cm_4096_fp64_full_size():
     _check(W.baseline_config(4), steps=3)
+
+
+def test_config4_cm_4096_fp64_full_size_with_an_arrested_step():
+    # The first arrest of config 4 is step 1226, so the 3-step test above never takes kernel Y's
+    # arrested branch (vh = 0, a2 := a1, the skipped TMA boxes) at full size.  Start instead with
+    # the uphill velocity v = -0.06 a(phi) (computed by the oracle): step 1 raises the energy, is
+    # logged, and step 2 runs the arrested branch on all 4096 x 4096 sites.
+    w = W.baseline_config(4)
+    m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=w.B, K=w.K)
+    vel = (-0.06 * oracle.accel(m, w.fields[0]))[None]
+    s = _check(w, steps=3, vel=vel)
+    assert s.arrests(0)[0][:1] == [1]
 
 
 def test_config4_cm_4096_full_size_verlet():

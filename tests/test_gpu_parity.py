@@ -40,15 +40,15 @@ def _dev(a, dtype=torch.float64):
 
 
 def _run_parity(w, checkpoints=CHECKPOINTS, flags=0, field_tol=1e-11, lattices=None,
-                integrator="rk4"):
+                integrator="rk4", vel=None):
     ss = _ss()
     s = ss.solver_for(w, flags=flags, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
-    s.set_fields(_dev(w.fields))
+    s.set_fields(_dev(w.fields), None if vel is None else _dev(vel))
     lattices = range(w.batch) if lattices is None else lattices
     flows = {}
     for b in lattices:
         fl = oracle.Flow(_model(w, b), w.dt, integrator=integrator)
-        fl.set_fields(w.fields[b])
+        fl.set_fields(w.fields[b], None if vel is None else vel[b])
         flows[b] = fl
     E0 = s.energy()
     Q0 = s.charge()
@@ -119,6 +119,66 @@ def test_batched_sweep_per_lattice_arrests():
     assert len(set(logs)) > 1            # different B -> different arrest histories
 
 
+def test_batched_abelian_higgs():
+    # batch dimension x C = 4 template path: three lattices with their own vortex positions
+    ws = [W.ah_vortices(N=100, h=0.1, lam=1.0, count=2, min_sep=2.0, config=3 + 10 * k)
+          for k in range(3)]
+    w = ws[0]
+    w.fields = np.concatenate([x.fields for x in ws], axis=0)
+    w.batch = 3
+    _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50))
+
+
+def test_batched_dmi_table_with_per_lattice_B():
+    # general-DMI kernels (kCMG) x batch x B_batch
+    w = W.cm_sweep(batch=4, N=96)
+    w.dmi = W.DMI_NEEL
+    s, flows = _run_parity(w, checkpoints=(1, 2, 5, 10, 20, 50))
+    assert len(set(s.energy())) == w.batch               # different B -> different lattices
+
+
+def test_batched_fp32_with_per_lattice_B():
+    # packed fp32 kernels x batch x B_batch: energies within 1e-4 of the fp64 oracle per lattice
+    ss = _ss()
+    w = W.cm_sweep(batch=5, N=96)
+    s = ss.solver_for(w, dtype=ss.F32)
+    s.set_fields(_dev(w.fields, torch.float32))
+    flows = []
+    for b in range(w.batch):
+        fl = oracle.Flow(_model(w, b), w.dt)
+        fl.set_fields(w.fields[b])
+        flows.append(fl)
+    for _ in range(3):
+        s.step(40)
+        E, Q = s.energy(), s.charge()
+        for b, fl in enumerate(flows):
+            fl.step(40)
+            assert abs(E[b] - fl.energy) <= 1e-4 * _floor(fl.m, fl.get_fields()[0], fl.energy), b
+            assert abs(Q[b] - fl.charge) <= 1e-4
+    assert len(set(E)) == w.batch
+
+
+def test_arrested_steps_from_an_uphill_velocity():
+    # kernel Y's arrested branch (vh = 0, a2 := a1) right at steps 2.. on a ragged lattice: start
+    # with v = -c a(phi) (uphill, from the oracle) so that step 1 is logged
+    w = W.cm_quench(N=190)
+    vel = (-0.06 * oracle.accel(_model(w), w.fields[0]))[None]
+    s, flows = _run_parity(w, checkpoints=(1, 2, 3, 5, 10), vel=vel)
+    assert flows[0].arrests()[:1] == [1]
+
+
+def test_extreme_aspect_ratios_at_the_size_limits():
+    # widest and tallest lattices the reduction tree supports (include/ss.h "Limits"): Nx = 65536
+    # (1024 segment partials per row) and Ny = 32768 (32 rows per thread in the y-tree)
+    for Nx, Ny in ((65536, 6), (8, 32768)):
+        rng = np.random.default_rng(Nx + Ny)
+        f = rng.standard_normal((1, 3, Ny, Nx))
+        f /= np.sqrt((f * f).sum(1, keepdims=True))
+        f[:, :, ~W.interior_mask(Nx, Ny)] = np.array([0.0, 0.0, 1.0])[None, :, None]
+        w = W.Workload("limit", W.CM, Nx, Ny, 0.2, 0.1, kappa=1.0, B=0.6, K=0.1, fields=f)
+        _run_parity(w, checkpoints=(1, 2))
+
+
 def test_verlet_cm_ragged_first_100_steps_with_arrests():
     # one-gradient-per-step integrator (DESIGN R15), same tolerances; config-1 recipe on a ragged
     # lattice; the first arrests fall inside the window
@@ -161,8 +221,6 @@ def test_verlet_fp32_and_graph_vs_direct():
         outs.append((f.cpu(), v.cpu(), s.energy(), s.charge(), s.arrests(0)))
     assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
     assert outs[0][2:] == outs[1][2:]
-    with pytest.raises(ss.SSError):
-        ss.solver_for(w, flags=ss.FLAG_STAGED, integrator=ss.VERLET)   # no staged Verlet
 
 
 @pytest.mark.parametrize("table", ["neel", "d2d", "random", "bloch"])
@@ -333,6 +391,14 @@ def test_error_paths():
     assert e.value.code == ss.ERR_ARG
     with pytest.raises(ss.SSError):
         ss.Solver(7, 64, 64, 0.2)                      # unknown theory
+    for kw in (dict(Nx=65538, Ny=64), dict(Nx=64, Ny=32770), dict(Nx=64, Ny=64, batch=65536)):
+        with pytest.raises(ss.SSError) as e:           # over a limit of this build (ss.h "Limits")
+            ss.Solver(0, kw["Nx"], kw["Ny"], 0.2, batch=kw.get("batch", 1))
+        assert e.value.code == ss.ERR_UNSUPPORTED
+        assert ss.workspace_bytes(0, kw["Nx"], kw["Ny"], batch=kw.get("batch", 1)) == 0
+    with pytest.raises(ss.SSError) as e:
+        ss.Solver(0, 64, 64, 0.2, flags=2)             # unknown flag bit
+    assert e.value.code == ss.ERR_ARG
     s = ss.Solver(0, 64, 64, 0.2, kappa=1.0, B=0.6)
     with pytest.raises(ss.SSError) as e:
         s.step(1)                                      # before set_fields

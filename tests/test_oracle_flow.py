@@ -64,6 +64,35 @@ def test_rk4_order_unconstrained():
     assert 24.0 < drifts[0] / drifts[1] < 40.0
 
 
+def test_constrained_scheme_is_first_order_in_dt():
+    """SURVEY 8(c6) "Constrained scheme ... error ratio ~2" (survey scratch: 2.02).  Chiral magnet
+    from rest, no arrest inside the window, fixed final time: with the projection of
+    PAPER.md:129+154 applied to every stage field and stage gradient and NO centripetal term
+    (DESIGN R7) the RK4 stages are consistent only to first order on the sphere, so field and
+    velocity errors halve with dt -- where the unconstrained theory shows ~16
+    (test_rk4_order_unconstrained).  A different placement of the projections (projecting only
+    the final field, or adding the -|v|^2 n term) changes this order."""
+    w = W.cm_single(N=32, noise=0.0)
+    m = oracle.model(oracle.CM, 32, 32, w.h, kappa=1.0, B=0.6)
+    T = 0.2
+
+    def run(dt):
+        fl = oracle.Flow(m, dt)
+        fl.set_fields(w.fields[0])
+        fl.step(round(T / dt))
+        assert fl.scalars()["n_arrests"] == 0
+        return fl.get_fields()
+    ref, vref = run(T / 512)
+    ef, ev = [], []
+    for dt in (T / 4, T / 8, T / 16, T / 32):
+        phi, vel = run(dt)
+        ef.append(np.abs(phi - ref).max())
+        ev.append(np.abs(vel - vref).max())
+    for e in (ef, ev):
+        for a, b in zip(e, e[1:]):
+            assert 1.8 < a / b < 2.4, (ef, ev)
+
+
 def test_newton_flow_is_second_order_in_time_from_rest():
     # phi(dt) - phi(0) = -dt^2/2 G + O(dt^4) from rest (eq. 3): catches a wrong mass / sign
     w = W.ah_vortices(N=20, h=0.2, lam=1.0, noise=0.05, centres=[(0.0, 0.0)])

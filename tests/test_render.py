@@ -67,3 +67,28 @@ def test_render_matches_cpu_restatement(case):
     assert fields_after.shape == phi.shape
     if not f32:
         assert np.abs(s.get_fields()[0].cpu().numpy()[0] - fl.get_fields()[0]).max() <= 1e-11
+
+
+@pytest.mark.gpu
+def test_render_marks_non_finite_interior_values():
+    # a NaN at an interior site is not the halo: it is drawn opaque magenta, stays out of the
+    # extrema, and the call reports SS_ERR_NONFINITE; the halo is found by position
+    import torch
+    from paper_2603_24370_b200 import ss
+    w = W.cm_single(N=64)
+    f = w.fields.copy()
+    f[0, 2, 30, 17] = np.nan
+    s = ss.solver_for(w)
+    s.set_fields(torch.from_numpy(f).to("cuda:0"))
+    with pytest.raises(ss.SSError) as e:
+        s.render(ss.OBS_ORDER)
+    assert e.value.code == ss.ERR_NONFINITE
+    img, (mn, mx) = s.render(ss.OBS_ORDER, strict=False)
+    got = img.cpu().numpy()
+    assert tuple(got[30, 17]) == (255, 0, 255, 255)
+    ok = np.isfinite(f[0, 2]) & W.interior_mask(64, 64)
+    assert (mn, mx) == (f[0, 2][ok].min(), f[0, 2][ok].max())
+    assert (got[~W.interior_mask(64, 64)] == 0).all() and (got[ok][:, 3] == 255).all()
+    vals = np.where(ok, f[0, 2], np.nan)
+    want, _ = oracle.colormap(vals)
+    assert (got[ok] == want[ok]).all()
