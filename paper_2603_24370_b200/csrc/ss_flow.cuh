@@ -29,6 +29,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "ss_theory.cuh"
 
 namespace ss {
@@ -226,10 +228,12 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     for (int c = 0; c < 2 * C; ++c) keep_new[k][c] = keep_old[k][c] = vreal(real(0));
 
   // raw site (row, lx) of chunk f -> the two stage fields in the rings
-  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, vreal* keep) {
+  // (edge_tag = false_type: the caller knows the site is interior, no test is compiled)
+  auto fill_site = [&](const unsigned char* st, int f, int row, int lx, vreal* keep, auto edge_tag) {
     constexpr int RW = Cfg::RAWW;
     const int gx = x0 - HALO + lx, gy = f * FR + row;
-    const bool inter = gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
+    const bool inter = !decltype(edge_tag)::value ||
+                       (gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO);
     const int ro = row * RW + lx + (Cfg::XPAD - HALO);
     const real* rphi = reinterpret_cast<const real*>(st);
     const real* rvel = reinterpret_cast<const real*>(st + Cfg::ARRB);
@@ -296,16 +300,22 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   const bool xin = gx >= HALO && gx < Nx - HALO;
   const bool xedge = gx < 2 * HALO || gx >= Nx - 2 * HALO;
 
-  for (int f = f0; f <= ce; ++f) {
-    if (f <= f1) {
+  // One iteration of the march: fill chunk f, barrier, stencils of chunk f - 1.  EDGE = false is
+  // the steady state of a strip away from the lattice edge: chunk f is filled and chunk f - 1
+  // evaluated, every site involved is interior and at least 4 sites from the halo, so no
+  // per-site test exists and the sites of a thread are straight-line code that the compiler
+  // interleaves.  EDGE = true keeps every test (edge strips, first / last chunks of a segment).
+  auto iteration = [&](const int f, auto edge_tag) {
+    constexpr bool EDGE = decltype(edge_tag)::value;
+    if (!EDGE || f <= f1) {
       const int k = f - f0;
       const unsigned char* st = smem + (k % NST) * Cfg::STAGEB;
       mbar_wait(&full[k % NST], (uint32_t)((k / NST) & 1));
 #pragma unroll
-      for (int k2 = 0; k2 < SPT; ++k2) fill_site(st, f, r0 + k2, tx + HALO, keep_new[k2]);
+      for (int k2 = 0; k2 < SPT; ++k2) fill_site(st, f, r0 + k2, tx + HALO, keep_new[k2], edge_tag);
       if (tid < 4 * FR / VEC) {  // the x-halo columns 0, 1, FW+2, FW+3 of the chunk's rows
         const int q = tid % (4 / VEC) * VEC;
-        fill_site(st, f, tid / (4 / VEC), q < 2 ? q : FW + q, nullptr);
+        fill_site(st, f, tid / (4 / VEC), q < 2 ? q : FW + q, nullptr, edge_tag);
       }
     }
     __syncthreads();
@@ -313,7 +323,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 
     const int sc = f - 1;
     if (sc - 1 >= cs && sc - 1 < ce) flush_partials(sc - 1, (f - 1) & 1);
-    if (sc >= cs && sc < ce) {
+    if (!EDGE || (sc >= cs && sc < ce)) {
       const int gy0 = sc * FR + r0;
       // ring offsets of rows gy0-2 .. gy0+SPT+1 at the thread's column
       int rw[SPT + 4];
@@ -340,7 +350,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         s0[k] = s1[k] = s2[k] = 0.0;
-        act[k] = xin && gy0 + k >= HALO && gy0 + k < Ny - HALO;
+        act[k] = !EDGE || (xin && gy0 + k >= HALO && gy0 + k < Ny - HALO);
       }
       const long long o = (long long)b * C * p.plane + (long long)gy0 * Nx + gx;
       real* o0 = p.out0 + o;
@@ -379,7 +389,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
           auto TA = [&](int c, int dy, int dx) -> vreal { return tile(ringA, col, rw, c, k + dy + 2, dx); };
           if (KIND == KX || KIND == KV) {
             vreal e, q;
-            if (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
+            if (EDGE && (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO)) {
               if constexpr (AHXY) Th::accel_xy(TA, p, Bz, xy[k][0], xy[k][1], aA[k]);
               else Th::accel(TA, p, Bz, aA[k]);
               if constexpr (VEC == 2) Th::densities(TA, p, Bz, EdgeW2(gx, gy, Nx, Ny), e, q);
@@ -479,6 +489,15 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     for (int k = 0; k < SPT; ++k)
 #pragma unroll
       for (int c = 0; c < 2 * C; ++c) keep_old[k][c] = keep_new[k][c];
+  };
+
+  // strips whose columns (x-halo included) are all >= 4 sites from the lattice edge
+  const bool inner_strip = x0 >= 2 * HALO + HALO && x0 + FW + HALO <= Nx - 2 * HALO;
+  for (int f = f0; f <= ce; ++f) {
+    const bool steady = inner_strip && f <= f1 && f - 1 >= cs && f - 1 < ce &&
+                        (f - 1) * FR >= 2 * HALO && f * FR + FR <= Ny - 2 * HALO;
+    if (steady) iteration(f, std::false_type{});
+    else iteration(f, std::true_type{});
   }
   __syncthreads();
   if (ce - 1 >= cs) flush_partials(ce - 1, ce & 1);

@@ -23,11 +23,11 @@ def _floor(m, phi, E):
     return max(abs(E), m.h * m.h * float(np.abs(de).sum()), 1e-300)
 
 
-def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4", vel=None):
+def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4", vel0=None):
     ss = _ss()
     s = ss.solver_for(w, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
     s.set_fields(torch.from_numpy(w.fields).to("cuda:0"),
-                 None if vel is None else torch.from_numpy(vel).to("cuda:0"))
+                 None if vel0 is None else torch.from_numpy(vel0).to("cuda:0"))
     s.step(steps)
     phi, vel = s.get_fields()
     E, Q, KE = s.energy(), s.charge(), s.kinetic()
@@ -37,7 +37,7 @@ def _check(w, steps, lattices=(0,), dtype=None, field_tol=1e-11, integrator="rk4
         B = w.B if w.B_batch is None else float(w.B_batch[b])
         m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K, lam=w.lam)
         fl = oracle.Flow(m, w.dt, integrator=integrator)
-        fl.set_fields(w.fields[b], None if vel is None else vel[b])
+        fl.set_fields(w.fields[b], None if vel0 is None else vel0[b])
         fl.step(steps)
         ophi, ovel = fl.get_fields()
         gp, gv = phi[b].cpu().numpy(), vel[b].cpu().numpy()
@@ -74,7 +74,7 @@ def test_config4_cm_4096_fp64_full_size_with_an_arrested_step():
     w = W.baseline_config(4)
     m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=w.B, K=w.K)
     vel = (-0.06 * oracle.accel(m, w.fields[0]))[None]
-    s = _check(w, steps=3, vel=vel)
+    s = _check(w, steps=3, vel0=vel)
     assert s.arrests(0)[0][:1] == [1]
 
 

@@ -40,15 +40,15 @@ def _dev(a, dtype=torch.float64):
 
 
 def _run_parity(w, checkpoints=CHECKPOINTS, flags=0, field_tol=1e-11, lattices=None,
-                integrator="rk4", vel=None):
+                integrator="rk4", vel0=None):
     ss = _ss()
     s = ss.solver_for(w, flags=flags, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
-    s.set_fields(_dev(w.fields), None if vel is None else _dev(vel))
+    s.set_fields(_dev(w.fields), None if vel0 is None else _dev(vel0))
     lattices = range(w.batch) if lattices is None else lattices
     flows = {}
     for b in lattices:
         fl = oracle.Flow(_model(w, b), w.dt, integrator=integrator)
-        fl.set_fields(w.fields[b], None if vel is None else vel[b])
+        fl.set_fields(w.fields[b], None if vel0 is None else vel0[b])
         flows[b] = fl
     E0 = s.energy()
     Q0 = s.charge()
@@ -163,7 +163,7 @@ def test_arrested_steps_from_an_uphill_velocity():
     # with v = -c a(phi) (uphill, from the oracle) so that step 1 is logged
     w = W.cm_quench(N=190)
     vel = (-0.06 * oracle.accel(_model(w), w.fields[0]))[None]
-    s, flows = _run_parity(w, checkpoints=(1, 2, 3, 5, 10), vel=vel)
+    s, flows = _run_parity(w, checkpoints=(1, 2, 3, 5, 10), vel0=vel)
     assert flows[0].arrests()[:1] == [1]
 
 
