@@ -86,7 +86,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index, period=0.002):
         super().__init__(daemon=True)
         self.index, self.period = index, period
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.power, self.reasons, self.max_mhz = [], [], set(), None
         self._stop_evt = threading.Event()
         try:
             import pynvml
@@ -112,6 +112,7 @@ class ClockSampler(threading.Thread):
         while not self._stop_evt.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) * 1e-3)
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 for bit, nm in names.items():
                     if r & bit:
@@ -124,8 +125,10 @@ class ClockSampler(threading.Thread):
         self._stop_evt.set()
         self.join(timeout=2.0)
         s = sorted(self.samples)
+        pw = sorted(self.power)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
-                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s),
+                "power_w": pw[len(pw) // 2] if pw else None, "power_w_max": pw[-1] if pw else None}
 
 
 def nvml_index(torch, dev):
