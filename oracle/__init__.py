@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-CM, AH = 0, 1
+CM, AH, BS = 0, 1, 2
+POT_STANDARD, POT_EASY_PLANE, POT_BROKEN = 0, 1, 2
 _dp = C.POINTER(C.c_double)
 
 
@@ -33,7 +34,8 @@ def build(force: bool = False) -> str:
 class _Model(C.Structure):
     _fields_ = [("theory", C.c_int), ("Nx", C.c_int), ("Ny", C.c_int), ("h", C.c_double),
                 ("kappa", C.c_double), ("B", C.c_double), ("K", C.c_double),
-                ("lam", C.c_double), ("dmi", C.c_int), ("d", C.c_double * 6)]
+                ("lam", C.c_double), ("dmi", C.c_int), ("d", C.c_double * 6),
+                ("pot", C.c_int), ("potN", C.c_int), ("mu", C.c_double)]
 
 
 _lib = None
@@ -54,6 +56,8 @@ def lib():
         L.orc_cm_energy_bond_d.restype = C.c_double
         L.orc_ah_energy_bond.argtypes = [_dp, C.c_int, C.c_int, C.c_double, C.c_double]
         L.orc_ah_energy_bond.restype = C.c_double
+        L.orc_bs_energy_plain.argtypes = [C.POINTER(_Model), _dp]
+        L.orc_bs_energy_plain.restype = C.c_double
         L.orc_energy_charge.argtypes = [C.POINTER(_Model), _dp, C.c_int, _dp, _dp, _dp, _dp]
         L.orc_gradient.argtypes = [C.POINTER(_Model), _dp, _dp]
         L.orc_accel.argtypes = [C.POINTER(_Model), _dp, _dp]
@@ -89,14 +93,18 @@ def threads() -> int:
 
 
 def ncomp(theory: int) -> int:
-    return 3 if theory == CM else 4
+    return 4 if theory == AH else 3
 
 
-def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None):
+def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None, mu=0.0,
+          pot=POT_STANDARD, potN=3):
     """dmi: None = kappa n.(curl n) (BASELINE), else the six numbers (d_x, d_y) of
-    PAPER.md:196 eq. (5): e_DMI = kappa sum_mu d_mu . (n x d_mu n)."""
+    PAPER.md:196 eq. (5): e_DMI = kappa sum_mu d_mu . (n x d_mu n).
+    Baby Skyrme (theory BS): kappa = Skyrme coupling, V proportional to mu^2,
+    pot in POT_*, potN = N of the Z_N-symmetric "broken" potential."""
     m = _Model(int(theory), int(Nx), int(Ny), float(h), float(kappa), float(B), float(K),
                float(lam))
+    m.pot, m.potN, m.mu = int(pot), int(potN), float(mu)
     if dmi is not None:
         m.dmi = 1
         m.d = (C.c_double * 6)(*[float(x) for x in np.asarray(dmi).reshape(6)])
@@ -125,6 +133,8 @@ def tree_sum2d(v):
 def energy_bond(m, f):
     """Plain bond-sum definition of E_h (straight summation)."""
     f = _f64(f)
+    if m.theory == BS:
+        return lib().orc_bs_energy_plain(C.byref(m), _p(f))
     if m.theory == CM:
         if m.dmi:
             d = np.array(list(m.d))
@@ -231,7 +241,7 @@ def observable(m, f, which):
     out = np.full((m.Ny, m.Nx), np.nan)
     I = (slice(2, m.Ny - 2), slice(2, m.Nx - 2))
     if which == 2:
-        v = f[2] if m.theory == CM else np.sqrt(f[0] * f[0] + f[1] * f[1])
+        v = np.sqrt(f[0] * f[0] + f[1] * f[1]) if m.theory == AH else f[2]
     else:
         _, _, de, dq = energy_charge(m, f, densities=True)
         v = de if which == 0 else dq

@@ -23,8 +23,11 @@
  *   cm/ah gradients brute-force central differences of the bond-form energy (8x8)
  *   charges         integer degree of seeded ansaetze; unit flux of a vortex
  *   flow            RK4 order on AH; |n|=1, v.n=0; arrest invariants; Bogomolny bound
- *   parity unpinned: the placement of the projections inside the RK4 stages
- *   (DESIGN R7) has no external pin beyond those order/invariant checks.
+ *   baby Skyrme     brute-force gradient (12x12, radius-4 exact gradient), plain == site form,
+ *                   vacuum, closed-form E4 / E0 of the hedgehog (1-D quadrature), Belavin-Polyakov
+ *                   lump E2 = 4 pi, Derrick scaling and the virial E4 = E0 at the relaxed minimum
+ *   parity unpinned: the placement of the projections inside the RK4 stages (DESIGN R7) is
+ *   fixed by definition; its order of convergence is pinned (error ratio ~2).
  */
 #include <math.h>
 #include <omp.h>
@@ -34,7 +37,8 @@
 
 #define PI 3.14159265358979323846
 
-enum { ORC_CM = 0, ORC_AH = 1 };
+enum { ORC_CM = 0, ORC_AH = 1, ORC_BS = 2 };
+enum { ORC_POT_STANDARD = 0, ORC_POT_EASY_PLANE = 1, ORC_POT_BROKEN = 2 };
 
 static inline size_t at(int Nx, int Ny, int c, int j, int i) {
   return ((size_t)c * Ny + j) * Nx + i;
@@ -458,9 +462,160 @@ typedef struct {
   double h, kappa, B, K, lambda;
   int dmi;       /* 0: kappa n.(curl n) (BASELINE, d_mu = -e_mu); 1: the table d below */
   double d[6];   /* d_x, d_y of PAPER.md:196 eq. (5) */
+  int pot, potN; /* baby Skyrme: potential (ORC_POT_*), and N of the Z_N-symmetric one */
+  double mu;     /* baby Skyrme: V is proportional to mu^2 */
 } orc_model;
 
-static int ncomp(int theory) { return theory == ORC_CM ? 3 : 4; }
+static int ncomp(int theory) { return theory == ORC_AH ? 4 : 3; }
+static int unit_field(int theory) { return theory != ORC_AH; } /* |m| = 1 constraint */
+
+/* ------------------------------------------------------------------ baby Skyrme */
+/* Functional (Table 2; model list PAPER.md:90):
+ *   E_BS = int 1/2 |grad m|^2 + (kappa^2/4) |d_i m x d_j m|^2 + V(m),  m in S^2.
+ * The double sum over i, j in {1,2} of |d_i m x d_j m|^2 is 2 |d_1 m x d_2 m|^2, so the Skyrme
+ * term is (kappa^2/2) |d_1 m x d_2 m|^2.  Discrete energy (DESIGN R18):
+ *   - 1/2 |grad m|^2 exactly as the exchange term of the chiral magnet: bonds (i, j = i + k mu),
+ *     k in {1,2}, at least one end interior, J_k/2 |m_i - m_j|^2 (eq. 2 weights, DESIGN R1, R3);
+ *   - Skyrme term and potential as SITE sums over the interior with eq. (1):
+ *       h^2 sum_{i in I} [ (kappa^2/2) |D_x m x D_y m|_i^2 + V(m_i) ]
+ *     (the stencil of a halo site would reach outside the lattice; the term is quartic in
+ *     derivatives, so it vanishes with all its first variations on the vacuum and needs no
+ *     halo-bond closure to keep the wall force-free).
+ * Potentials (the paper names them, and prints no formula; these are the
+ * textbook forms with the vacuum m = e3 of the frozen halo; own parametrisation by mu^2):
+ *   standard    V = mu^2 (1 - m3)
+ *   easy plane  V = 1/2 mu^2 m1^2
+ *   broken      V = mu^2 |1 - (m1 + i m2)^N|^2 (1 - m3)       (Z_N-symmetric, N = potN >= 1)
+ * Exact gradient (DESIGN R2, R18): with a = D_x m, b = D_y m, w = a x b,
+ *   F_x = d e4/d a = kappa^2 (b x w),  F_y = d e4/d b = kappa^2 (w x a)   on I, 0 on the halo,
+ *   G = -(Lx + Ly) m - D_x F_x - D_y F_y + dV/dm        (radius 4: F needs radius 2, D F again). */
+static void cpow_int(double x, double y, int N, double* re, double* im) { /* (x + i y)^N */
+  double a = 1.0, b = 0.0;
+  for (int k = 0; k < N; ++k) {
+    double t = a * x - b * y;
+    b = a * y + b * x;
+    a = t;
+  }
+  *re = a;
+  *im = b;
+}
+static double bs_potential(const orc_model* m, double m1, double m2, double m3) {
+  const double mu2 = m->mu * m->mu;
+  if (m->pot == ORC_POT_STANDARD) return mu2 * (1.0 - m3);
+  if (m->pot == ORC_POT_EASY_PLANE) return 0.5 * mu2 * (m1 * m1);
+  double a, b;
+  cpow_int(m1, m2, m->potN, &a, &b);
+  return mu2 * ((1.0 - a) * (1.0 - a) + b * b) * (1.0 - m3);
+}
+static void bs_potential_grad(const orc_model* m, double m1, double m2, double m3, double dV[3]) {
+  const double mu2 = m->mu * m->mu;
+  if (m->pot == ORC_POT_STANDARD) { dV[0] = 0.0; dV[1] = 0.0; dV[2] = -mu2; return; }
+  if (m->pot == ORC_POT_EASY_PLANE) { dV[0] = mu2 * m1; dV[1] = 0.0; dV[2] = 0.0; return; }
+  /* z = m1 + i m2, P = 1 - z^N = (1-a) - i b;  d z^N/d m1 = N z^(N-1),  d z^N/d m2 = i N z^(N-1) */
+  double a, b, c, d;
+  const double N = (double)m->potN;
+  cpow_int(m1, m2, m->potN, &a, &b);
+  cpow_int(m1, m2, m->potN - 1, &c, &d);
+  const double P2 = (1.0 - a) * (1.0 - a) + b * b;
+  dV[0] = mu2 * (1.0 - m3) * (2.0 * (-(1.0 - a) * (N * c) + b * (N * d)));
+  dV[1] = mu2 * (1.0 - m3) * (2.0 * ((1.0 - a) * (N * d) + b * (N * c)));
+  dV[2] = -mu2 * P2;
+}
+/* w = D_x m x D_y m at a site whose radius-2 neighbours are in the lattice */
+static void bs_site_w(const double* f, int Nx, int Ny, int j, int i, double h, double a[3],
+                      double b[3], double w[3]) {
+  const size_t P = (size_t)Nx * Ny;
+  for (int c = 0; c < 3; ++c) {
+    a[c] = Dx(f + c * P, Nx, j, i, h);
+    b[c] = Dy(f + c * P, Nx, j, i, h);
+  }
+  w[0] = a[1] * b[2] - a[2] * b[1];
+  w[1] = a[2] * b[0] - a[0] * b[2];
+  w[2] = a[0] * b[1] - a[1] * b[0];
+}
+/* Plain definition: bond loop + site loop, straight summation. */
+double orc_bs_energy_plain(const orc_model* m, const double* f) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  const double h = m->h;
+  const size_t P = (size_t)Nx * Ny;
+  double E = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t s = (size_t)j * Nx + i;
+      for (int mu = 0; mu < 2; ++mu)
+        for (int k = 1; k <= 2; ++k) {
+          int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+          if (!inside(Nx, Ny, i2, j2)) continue;
+          if (!interior(Nx, Ny, i, j) && !interior(Nx, Ny, i2, j2)) continue;
+          size_t t = (size_t)j2 * Nx + i2;
+          double d1r = f[s] - f[t], d2r = f[P + s] - f[P + t], d3r = f[2 * P + s] - f[2 * P + t];
+          E += 0.5 * Jw[k] * (d1r * d1r + d2r * d2r + d3r * d3r);
+        }
+      if (interior(Nx, Ny, i, j)) {
+        double a[3], b[3], w[3];
+        bs_site_w(f, Nx, Ny, j, i, h, a, b, w);
+        E += (h * h) * (0.5 * (m->kappa * m->kappa) * (w[0] * w[0] + w[1] * w[1] + w[2] * w[2]) +
+                        bs_potential(m, f[s], f[P + s], f[2 * P + s]));
+      }
+    }
+  return E;
+}
+/* Site form: e_i = sum_mu sum_k w(j) J_|k|/(4h^2) |m_i - m_j|^2 + (kappa^2/2)|w_i|^2 + V(m_i). */
+static double bs_site_energy(const orc_model* m, const double* f, int j, int i) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  const double h = m->h;
+  const size_t P = (size_t)Nx * Ny;
+  static const int ks[4] = {1, -1, 2, -2};
+  size_t s = (size_t)j * Nx + i;
+  double e = 0.0;
+  for (int mu = 0; mu < 2; ++mu)
+    for (int q = 0; q < 4; ++q) {
+      int k = ks[q], ak = k < 0 ? -k : k;
+      int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+      size_t t = (size_t)j2 * Nx + i2;
+      double wt = interior(Nx, Ny, i2, j2) ? 1.0 : 2.0;
+      double d1r = f[s] - f[t], d2r = f[P + s] - f[P + t], d3r = f[2 * P + s] - f[2 * P + t];
+      e += wt * (Jw[ak] / (4.0 * (h * h)) * (d1r * d1r + d2r * d2r + d3r * d3r));
+    }
+  double a[3], b[3], w[3];
+  bs_site_w(f, Nx, Ny, j, i, h, a, b, w);
+  e += 0.5 * (m->kappa * m->kappa) * (w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+  e += bs_potential(m, f[s], f[P + s], f[2 * P + s]);
+  return e;
+}
+/* Flux arrays F_x, F_y ([3][Ny][Nx] each): d e4 / d(D_mu m) on I, 0 on the halo. */
+static void bs_flux(const orc_model* m, const double* f, double* Fx, double* Fy) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  const size_t P = (size_t)Nx * Ny;
+  const double k2 = m->kappa * m->kappa;
+  memset(Fx, 0, 3 * P * sizeof(double));
+  memset(Fy, 0, 3 * P * sizeof(double));
+#pragma omp parallel for schedule(static)
+  for (int j = 2; j < Ny - 2; ++j)
+    for (int i = 2; i < Nx - 2; ++i) {
+      double a[3], b[3], w[3];
+      bs_site_w(f, Nx, Ny, j, i, m->h, a, b, w);
+      size_t s = (size_t)j * Nx + i;
+      Fx[s] = k2 * (b[1] * w[2] - b[2] * w[1]);           /* b x w */
+      Fx[P + s] = k2 * (b[2] * w[0] - b[0] * w[2]);
+      Fx[2 * P + s] = k2 * (b[0] * w[1] - b[1] * w[0]);
+      Fy[s] = k2 * (w[1] * a[2] - w[2] * a[1]);           /* w x a */
+      Fy[P + s] = k2 * (w[2] * a[0] - w[0] * a[2]);
+      Fy[2 * P + s] = k2 * (w[0] * a[1] - w[1] * a[0]);
+    }
+}
+static void bs_site_gradient(const orc_model* m, const double* f, const double* Fx, const double* Fy,
+                             int j, int i, double G[3]) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  const double h = m->h;
+  const size_t P = (size_t)Nx * Ny;
+  size_t s = (size_t)j * Nx + i;
+  double dV[3];
+  bs_potential_grad(m, f[s], f[P + s], f[2 * P + s], dV);
+  for (int c = 0; c < 3; ++c)
+    G[c] = -(Lx(f + c * P, Nx, j, i, h) + Ly(f + c * P, Nx, j, i, h)) -
+           (Dx(Fx + c * P, Nx, j, i, h) + Dy(Fy + c * P, Nx, j, i, h)) + dV[c];
+}
 
 /* Energy and charge with the canonical tree (DESIGN R10): E = (h*h) * tree(e_i),
  * halo sites contribute +0.0.  dens_e / dens_q (Ny*Nx each) may be NULL.
@@ -482,6 +637,9 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
         e[a] = m->dmi ? cm_site_energy_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d)
                       : cm_site_energy(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K);
         q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h);
+      } else if (m->theory == ORC_BS) {
+        e[a] = bs_site_energy(m, f, j, i);
+        q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h); /* the same degree density */
       } else {
         e[a] = which_energy ? ah_site_energy_literal(f, Nx, Ny, j, i, m->h, m->lambda)
                             : ah_site_energy(f, Nx, Ny, j, i, m->h, m->lambda);
@@ -497,19 +655,30 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
 /* Raw gradient G on the interior (halo entries 0), [C][Ny][Nx]. */
 void orc_gradient(const orc_model* m, const double* f, double* G) {
   const int Nx = m->Nx, Ny = m->Ny, C = ncomp(m->theory);
+  double *Fx = NULL, *Fy = NULL;
+  if (m->theory == ORC_BS) {
+    Fx = (double*)malloc(3 * (size_t)Nx * Ny * sizeof(double));
+    Fy = (double*)malloc(3 * (size_t)Nx * Ny * sizeof(double));
+    bs_flux(m, f, Fx, Fy);
+  }
 #pragma omp parallel for schedule(static)
   for (int j = 0; j < Ny; ++j)
     for (int i = 0; i < Nx; ++i) {
       double g[4] = {0, 0, 0, 0};
       if (interior(Nx, Ny, i, j)) {
-        if (m->theory == ORC_CM)
+        if (m->theory == ORC_CM) {
           if (m->dmi) cm_site_gradient_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d, g);
           else cm_site_gradient(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, g);
-        else
+        } else if (m->theory == ORC_BS) {
+          bs_site_gradient(m, f, Fx, Fy, j, i, g);
+        } else {
           ah_site_gradient(f, Nx, Ny, j, i, m->h, m->lambda, g);
+        }
       }
       for (int c = 0; c < C; ++c) G[at(Nx, Ny, c, j, i)] = g[c];
     }
+  free(Fx);
+  free(Fy);
 }
 
 /* Acceleration a = -Pi_f(G(f)) on the interior (eq. (3) with the tangent
@@ -521,7 +690,7 @@ void orc_accel(const orc_model* m, const double* f, double* a) {
 #pragma omp parallel for schedule(static)
   for (int j = 2; j < Ny - 2; ++j)
     for (int i = 2; i < Nx - 2; ++i) {
-      if (m->theory == ORC_CM) {
+      if (unit_field(m->theory)) {
         double g1 = a[at(Nx, Ny, 0, j, i)], g2 = a[at(Nx, Ny, 1, j, i)], g3 = a[at(Nx, Ny, 2, j, i)];
         double n1 = f[at(Nx, Ny, 0, j, i)], n2 = f[at(Nx, Ny, 1, j, i)], n3 = f[at(Nx, Ny, 2, j, i)];
         double gn = (g1 * n1 + g2 * n2) + g3 * n3;
@@ -632,7 +801,7 @@ static void stage_field(const orc_flow* s, double alpha, double beta, const doub
         mm[c] = s->phi[a] + alpha * vh;
         if (acc) mm[c] = mm[c] + beta * acc[a];
       }
-      if (s->m.theory == ORC_CM) {
+      if (unit_field(s->m.theory)) {
         double nn = sqrt((mm[0] * mm[0] + mm[1] * mm[1]) + mm[2] * mm[2]);
         for (int c = 0; c < 3; ++c) mm[c] = mm[c] / nn;
       }
@@ -661,7 +830,7 @@ void orc_flow_step(orc_flow* s, int64_t k) {
           f[c] = (s->phi[a] + dt * vh) + sdt2 * ((s->a1[a] + s->a2[a]) + s->a3[a]);
           u[c] = vh + sdt * ((s->a1[a] + 2.0 * s->a2[a]) + (2.0 * s->a3[a] + s->a4[a]));
         }
-        if (s->m.theory == ORC_CM) {
+        if (unit_field(s->m.theory)) {
           double nn = sqrt((f[0] * f[0] + f[1] * f[1]) + f[2] * f[2]);
           for (int c = 0; c < 3; ++c) f[c] = f[c] / nn;
           double un = (u[0] * f[0] + u[1] * f[1]) + u[2] * f[2];
@@ -708,7 +877,7 @@ void orc_flow_step_verlet(orc_flow* s, int64_t k) {
           s->a2[a] = w; /* scratch: the half-kicked velocity */
           mm[c] = s->phi[a] + dt * w;
         }
-        if (s->m.theory == ORC_CM) {
+        if (unit_field(s->m.theory)) {
           double nn = sqrt((mm[0] * mm[0] + mm[1] * mm[1]) + mm[2] * mm[2]);
           for (int c = 0; c < 3; ++c) mm[c] = mm[c] / nn;
         }
@@ -725,7 +894,7 @@ void orc_flow_step_verlet(orc_flow* s, int64_t k) {
           f[c] = s->s[a];
           u[c] = s->a2[a] + hdt * s->a4[a];
         }
-        if (s->m.theory == ORC_CM) {
+        if (unit_field(s->m.theory)) {
           double un = (u[0] * f[0] + u[1] * f[1]) + u[2] * f[2];
           for (int c = 0; c < 3; ++c) u[c] = u[c] - un * f[c];
         }

@@ -17,7 +17,8 @@ from dataclasses import dataclass, field
 import numpy as np
 
 SEED0 = 260324370
-CM, AH = 0, 1
+CM, AH, BS = 0, 1, 2
+POT_STANDARD, POT_EASY_PLANE, POT_BROKEN = 0, 1, 2   # baby-Skyrme potentials
 HALO = 2
 
 # DMI vectors (d_x, d_y) of PAPER.md:196 eq. (5), e_DMI = kappa sum_mu d_mu . (n x d_mu n)
@@ -41,6 +42,9 @@ class Workload:
     B: float = 0.0
     K: float = 0.0
     lam: float = 0.0
+    mu: float = 0.0                   # baby Skyrme: V proportional to mu^2
+    pot: int = 0                      # baby Skyrme: POT_*
+    potN: int = 3                     # baby Skyrme: N of the Z_N-symmetric potential
     batch: int = 1
     steps: int = 0
     B_batch: np.ndarray | None = None
@@ -49,7 +53,7 @@ class Workload:
 
     @property
     def C(self) -> int:
-        return 3 if self.theory == CM else 4
+        return 4 if self.theory == AH else 3
 
     @property
     def interior_sites(self) -> int:
@@ -191,6 +195,21 @@ def cm_sweep(batch=256, N=256, h=0.2, noise=0.01, config=5, steps=5000) -> Workl
         f[b] = _cm_finish(base.copy(), N, N, rng, noise)
     return Workload(f"cm_sweep_{batch}x{N}", CM, N, N, h, 0.5 * h, kappa=1.0, B=0.6, batch=batch,
                     steps=steps, B_batch=Bb, fields=f)
+
+
+def bs_single(N=128, h=0.2, kappa=1.0, mu=1.0, pot=POT_STANDARD, potN=3, noise=0.01, count=1,
+              config=6, steps=2000, batch=1, seed_offset=0) -> Workload:
+    """Baby skyrmions (SURVEY 8(f) NEXT-2b; not a BASELINE config): `count`
+    hedgehogs (the chiral-magnet ansatz, degree -1 each) at rejection-sampled centres (one:
+    centred) plus noise, renormalised; vacuum halo m = e3."""
+    rng = _rng(config, seed_offset)
+    L = N * h
+    f = np.empty((batch, 3, N, N))
+    for b in range(batch):
+        centres = [(0.0, 0.0)] if count == 1 else _reject_sample(rng, count, -L / 4, L / 4, 5.0)
+        f[b] = _cm_finish(skyrmion_ansatz(N, N, h, centres), N, N, rng, noise)
+    return Workload(f"bs_{N}_pot{pot}", BS, N, N, h, 0.5 * h, kappa=kappa, mu=mu, pot=pot, potN=potN,
+                    batch=batch, steps=steps, fields=f)
 
 
 def baseline_config(c: int, **kw) -> Workload:
