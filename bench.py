@@ -33,6 +33,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+THEORY_NAME = {0: "chiral_magnet", 1: "abelian_higgs", 2: "baby_skyrme"}
 METRIC = "lattice site-updates/s per flow step"
 UNIT = "site-updates/s"
 
@@ -44,6 +45,7 @@ WORKLOADS = {
     "ah2048_f64": ("ah_vortices", {}, "f64"),          # BASELINE configs[2], lambda = 1
     "sweep256_f64": ("cm_sweep", {}, "f64"),           # BASELINE configs[4], 256 lattices
     "cm64_f64": ("cm_single", {}, "f64"),              # BASELINE configs[0] (launch-bound)
+    "bs2048_f64": ("bs_bench", {}, "f64"),             # baby Skyrme (SURVEY 8(f) NEXT-2b)
 }
 
 
@@ -149,7 +151,8 @@ def time_oracle(w, seconds, lattices=None, integrator="rk4"):
     b = 0
     B = w.B if w.B_batch is None else float(w.B_batch[b])
     fl = oracle.Flow(oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B, K=w.K,
-                                  lam=w.lam), w.dt, integrator=integrator)
+                                  lam=w.lam, mu=w.mu, pot=w.pot, potN=w.potN), w.dt,
+                     integrator=integrator)
     fl.set_fields(w.fields[b])
     t0 = time.perf_counter()
     fl.step(1)
@@ -195,7 +198,8 @@ def run_reference(args):
     S = int((rate * budget) ** 0.5) // 64 * 64
     S = max(64, min(full, S))
     c = crop_workload(w, S)
-    fl = oracle.Flow(oracle.model(c.theory, S, S, c.h, kappa=c.kappa, B=c.B, K=c.K, lam=c.lam),
+    fl = oracle.Flow(oracle.model(c.theory, S, S, c.h, kappa=c.kappa, B=c.B, K=c.K, lam=c.lam,
+                                  mu=c.mu, pot=c.pot, potN=c.potN),
                      c.dt, integrator=args.integrator)
     fl.set_fields(c.fields[0])
     fl.step(args.warmup)
@@ -211,8 +215,8 @@ def run_reference(args):
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded)",
-        "config": {"workload": w.name, "sample": f"crop {S}x{S}", "theory":
-                   "chiral_magnet" if w.theory == 0 else "abelian_higgs", "h": w.h, "dt": w.dt},
+        "config": {"workload": w.name, "sample": f"crop {S}x{S}", "theory": THEORY_NAME[w.theory],
+                   "h": w.h, "dt": w.dt},
         "cpu_baseline": cpu,
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -227,6 +231,11 @@ KERNEL_UNITS = {
     "flow_x_grad_energy_charge_stage2": 4,    # reads phi', v'       -> writes a1, a2 (+ E, Q partials)
     # one-gradient-per-step integrator (--integrator verlet): reads phi, v, a -> phi', v', a'
     "flow_v_verlet_step_energy_charge_ke": 6,
+    # baby Skyrme: one tile kernel per RK4 stage (csrc/ss_bs.cuh)
+    "bs_stage2": 3,                       # reads phi, v             -> writes a2
+    "bs_stage3": 4,                       # reads phi, v, a1         -> writes a3
+    "bs_stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
+    "bs_stage1_grad_energy_charge": 2,    # reads phi'               -> writes a1 (+ E, Q partials)
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
@@ -464,10 +473,10 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms"] / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": r["dtname"], "data": "synthetic (seeded)",
-        "config": {"workload": w.name, "theory": "chiral_magnet" if w.theory == 0 else
-                   "abelian_higgs", "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
+        "config": {"workload": w.name, "theory": THEORY_NAME[w.theory], "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
                    "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
-                   "integrator": args.integrator, "schedule": "two-kernel",
+                   "integrator": args.integrator,
+                   "schedule": "per-stage tile kernels" if w.theory == 2 else "two-kernel",
                    "parallelism": f"replicas x{r['world']}",
                    "l2_policy": "working set (6 field arrays) larger than L2; no flush needed"
                    if 6 * r["field_bytes"] > 3 * 126e6 else

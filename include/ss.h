@@ -10,7 +10,10 @@
  *       SS_THEORY_CHIRAL_MAGNET  n in S^2:  1/2|grad n|^2 + kappa n.(curl n) + B(1-n3) + K(1-n3^2)
  *                                (PAPER.md:196 eq. 5, :327; DESIGN R1-R3),
  *       SS_THEORY_ABELIAN_HIGGS  phi in C, A in R^2: 1/2|D phi|^2 + 1/2 (curl A)^2
- *                                + (lambda/8)(1-|phi|^2)^2   (DESIGN R1-R3, R9);
+ *                                + (lambda/8)(1-|phi|^2)^2   (DESIGN R1-R3, R9),
+ *       SS_THEORY_BABY_SKYRME    m in S^2: 1/2|grad m|^2 + (kappa^2/2)|d1 m x d2 m|^2 + V(m)
+ *                                (DESIGN R18; SS_RK4 only, C = 3, charge =
+ *                                degree as for the chiral magnet);
  *   - the arrested Newton flow phi'' = -grad E_h (eq. 3) integrated with
  *     classical RK4, the unit-length projection applied in every stage
  *     (PAPER.md:129+154), the velocity set to zero whenever E_h rises (eq. 4);
@@ -46,7 +49,12 @@ extern "C" {
 
 typedef struct ss_solver ss_solver; /* opaque */
 
-enum { SS_THEORY_CHIRAL_MAGNET = 0, SS_THEORY_ABELIAN_HIGGS = 1 };
+enum { SS_THEORY_CHIRAL_MAGNET = 0, SS_THEORY_ABELIAN_HIGGS = 1, SS_THEORY_BABY_SKYRME = 2 };
+/* baby-Skyrme potentials (PAPER.md:90 names them, no formula is printed; DESIGN R18), vacuum e3:
+ *   SS_POT_STANDARD    V = mu^2 (1 - m3)
+ *   SS_POT_EASY_PLANE  V = 1/2 mu^2 m1^2
+ *   SS_POT_BROKEN      V = mu^2 |1 - (m1 + i m2)^N|^2 (1 - m3),  N = potential_n in 1..16 */
+enum { SS_POT_STANDARD = 0, SS_POT_EASY_PLANE = 1, SS_POT_BROKEN = 2 };
 enum { SS_F64 = 0, SS_F32 = 1 };
 enum {
   SS_OK = 0,
@@ -90,6 +98,9 @@ typedef struct {
   const double* dmi_d;     /* chiral magnet, optional HOST array[6] = (d_x, d_y): the DMI term   */
                            /* kappa sum_mu d_mu.(n x d_mu n) of PAPER.md:196 eq. (5) (DESIGN    */
                            /* R16).  NULL = kappa n.(curl n), i.e. d_x = -e_x, d_y = -e_y       */
+  double mu;               /* baby Skyrme: V is proportional to mu^2 (kappa = Skyrme coupling)   */
+  int potential;           /* baby Skyrme: SS_POT_*                                              */
+  int potential_n;         /* baby Skyrme: N of SS_POT_BROKEN                                    */
 } ss_params;
 
 /* Limits of this build: 5 <= Nx <= 65536, 5 <= Ny <= 32768 (the device-side reduction tree of

@@ -11,9 +11,10 @@
 #include <new>
 #include <vector>
 
+#include "ss_bs.cuh"
 #include "ss_flow.cuh"
-#include "ss_render.cuh"
 #include "ss_kernels.cuh"
+#include "ss_render.cuh"
 
 using namespace ss;
 
@@ -40,7 +41,8 @@ struct Layout {
   size_t part_bytes;   // one [batch][Ny][nseg] fp64 array
   size_t rows_bytes;   // [batch][3][Ny]
   size_t state_bytes, log_bytes, bb_bytes, render_bytes;
-  size_t off_phi[2], off_vel[2], off_a[2], off_part[3], off_rows, off_state, off_log, off_bb;
+  int nacc;            // acceleration arrays: a1, a2 (+ a3 for the baby-Skyrme stage kernels)
+  size_t off_phi[2], off_vel[2], off_a[3], off_part[3], off_rows, off_state, off_log, off_bb;
   size_t off_render;   // ss_render scratch: block extrema of one lattice, extrema, flag
   size_t total;
   int nseg;
@@ -56,7 +58,13 @@ bool supported_shape(int Nx, int Ny, const ss_params* p) {
 
 bool valid_shape(int theory, int Nx, int Ny, const ss_params* p) {
   if (!p) return false;
-  if (theory != SS_THEORY_CHIRAL_MAGNET && theory != SS_THEORY_ABELIAN_HIGGS) return false;
+  if (theory != SS_THEORY_CHIRAL_MAGNET && theory != SS_THEORY_ABELIAN_HIGGS &&
+      theory != SS_THEORY_BABY_SKYRME)
+    return false;
+  if (theory == SS_THEORY_BABY_SKYRME &&
+      (p->potential < SS_POT_STANDARD || p->potential > SS_POT_BROKEN ||
+       (p->potential == SS_POT_BROKEN && (p->potential_n < 1 || p->potential_n > 16))))
+    return false;
   if (p->dtype != SS_F64 && p->dtype != SS_F32) return false;
   if (Nx < 5 || Ny < 5 || p->batch < 1) return false;
   if (p->dtype == SS_F64 ? (Nx % 2 != 0) : (Nx % 4 != 0)) return false;
@@ -66,8 +74,9 @@ bool valid_shape(int theory, int Nx, int Ny, const ss_params* p) {
 
 Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
   Layout L;
-  const int C = theory == SS_THEORY_CHIRAL_MAGNET ? 3 : 4;
+  const int C = theory == SS_THEORY_ABELIAN_HIGGS ? 4 : 3;
   const size_t R = p->dtype == SS_F64 ? 8 : 4;
+  L.nacc = theory == SS_THEORY_BABY_SKYRME ? 3 : 2;  // the per-stage schedule stores a3 as well
   const size_t cap = p->arrest_log_capacity > 0 ? (size_t)p->arrest_log_capacity : 4096;
   L.nseg = (Nx + SEG - 1) / SEG;
   L.field_bytes = align_up((size_t)p->batch * C * Ny * Nx * R);
@@ -80,7 +89,7 @@ Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
   size_t o = 0;
   for (int i = 0; i < 2; ++i) { L.off_phi[i] = o; o += L.field_bytes; }
   for (int i = 0; i < 2; ++i) { L.off_vel[i] = o; o += L.field_bytes; }
-  for (int i = 0; i < 2; ++i) { L.off_a[i] = o; o += L.field_bytes; }
+  for (int i = 0; i < L.nacc; ++i) { L.off_a[i] = o; o += L.field_bytes; }
   for (int i = 0; i < 3; ++i) { L.off_part[i] = o; o += L.part_bytes; }
   L.off_rows = o; o += L.rows_bytes;
   L.off_state = o; o += L.state_bytes;
@@ -104,7 +113,8 @@ struct KernelNode {
 struct ss_solver {
   int theory, dtype, C, Nx, Ny, batch;
   int device, sms;  // the device the workspace lives on (current at ss_create) and its SM count
-  double h, dt, kappa, B, K, lambda;
+  double h, dt, kappa, B, K, lambda, mu;
+  int pot, potN;
   size_t R;
   cudaStream_t stream;
   char* ws;
@@ -122,6 +132,7 @@ struct ss_solver {
   std::vector<KernelNode> eval_nodes[2];  // X, row_reduce, finalize(advance = 0)
   cudaGraphExec_t step_exec[2];   // one flow step, per ping-pong parity
   cudaGraphExec_t multi_exec[2];  // MULTI consecutive steps in one graph (k steps per launch)
+  std::vector<unsigned char> consts;  // FlowArgs<real> holding the per-site constants (ss_render)
   std::vector<LatticeState> host_state;
   std::vector<double> Bb_host;  // per-lattice Zeeman field (host copy)
 
@@ -230,13 +241,35 @@ int flow_threads(int theory, int dtype, int kind) {
   return dtype == SS_F64 ? flow_threads_t<kAH, double>(kind) : flow_threads_t<kAH, float>(kind);
 }
 
+// per-site constants: time-step combinations, folded stencil weights, theory parameters
+template <typename real>
+void fill_constants(const ss_solver* s, FlowArgs<real>& a) {
+  const double dt = s->dt, h = s->h;
+  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg;
+  a.plane = (long long)s->Nx * s->Ny;
+  a.hdt = real(0.5 * dt); a.dt = real(dt);
+  a.qdt2 = real(0.25 * (dt * dt)); a.hdt2 = real(0.5 * (dt * dt));
+  a.sdt2 = real((dt * dt) / 6.0); a.sdt = real(dt / 6.0);
+  a.i12h = real(1.0 / (12.0 * h)); a.i12h2 = real(1.0 / (12.0 * h * h));
+  a.kappa = real(s->kappa); a.K = real(s->K); a.lambda = real(s->lambda);
+  a.lap0 = real(60.0 / (12.0 * h * h)); a.lap1 = real(16.0 / (12.0 * h * h));
+  a.lap2 = real(1.0 / (12.0 * h * h));
+  a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
+  a.K2 = real(2.0 * s->K);
+  a.jA = real((16.0 / 12.0) / (4.0 * h * h)); a.jB = real((-1.0 / 12.0) / (4.0 * h * h));
+  a.hk = real(s->kappa / (12.0 * h));
+  a.qs = real(1.0 / (4.0 * 3.14159265358979323846 * (12.0 * h) * (12.0 * h)));
+  for (int i = 0; i < 6; ++i) a.dk[i] = real(s->kappa / (12.0 * h) * s->dmi[i]);
+  a.bs_k2 = real(s->kappa * s->kappa); a.bs_mu2 = real(s->mu * s->mu);
+  a.bs_pot = s->pot; a.bs_potN = s->potN;
+}
+
 // kernel X (kind KX) evaluates the state in buffer `in`; kernels Y and V advance `in` -> `in ^ 1`
 // (V also a: acc(in) -> acc(in ^ 1))
 template <typename real>
 bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   FlowArgs<real> a;
   memset(&a, 0, sizeof(a));
-  const double dt = s->dt, h = s->h;
   if (!make_tmap(s, s->phi(in), &a.tm[0]) || !make_tmap(s, s->vel(in), &a.tm[1]) ||
       !make_tmap(s, s->acc(kind == KV ? in : 0), &a.tm[2]) || !make_tmap(s, s->acc(1), &a.tm[3]))
     return false;
@@ -252,21 +285,8 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   }
   a.state = s->state();
   a.Bb = (const double*)(s->ws + s->L.off_bb);
-  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg; a.cps = s->cps[kind];
-  a.plane = (long long)s->Nx * s->Ny;
-  a.hdt = real(0.5 * dt); a.dt = real(dt);
-  a.qdt2 = real(0.25 * (dt * dt)); a.hdt2 = real(0.5 * (dt * dt));
-  a.sdt2 = real((dt * dt) / 6.0); a.sdt = real(dt / 6.0);
-  a.i12h = real(1.0 / (12.0 * h)); a.i12h2 = real(1.0 / (12.0 * h * h));
-  a.kappa = real(s->kappa); a.K = real(s->K); a.lambda = real(s->lambda);
-  a.lap0 = real(60.0 / (12.0 * h * h)); a.lap1 = real(16.0 / (12.0 * h * h));
-  a.lap2 = real(1.0 / (12.0 * h * h));
-  a.dm1 = real(2.0 * s->kappa * 8.0 / (12.0 * h)); a.dm2 = real(2.0 * s->kappa / (12.0 * h));
-  a.K2 = real(2.0 * s->K);
-  a.jA = real((16.0 / 12.0) / (4.0 * h * h)); a.jB = real((-1.0 / 12.0) / (4.0 * h * h));
-  a.hk = real(s->kappa / (12.0 * h));
-  a.qs = real(1.0 / (4.0 * 3.14159265358979323846 * (12.0 * h) * (12.0 * h)));
-  for (int i = 0; i < 6; ++i) a.dk[i] = real(s->kappa / (12.0 * h) * s->dmi[i]);
+  fill_constants(s, a);
+  a.cps = s->cps[kind];
   KernelNode n;
   n.func = flow_func(s->ktheory, s->dtype, kind);
   const int NC = (s->Ny + FR - 1) / FR;
@@ -283,6 +303,60 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
 bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out)
                             : make_flow_node<float>(s, kind, in, out);
+}
+
+// baby Skyrme: one tile kernel per RK4 stage (ss_bs.cuh); stage 1 evaluates buffer `cur`,
+// stages 2-4 advance `cur` -> `cur ^ 1`
+template <typename real>
+void* bs_func(int stage) {
+  switch (stage) {
+    case 1: return (void*)bs_stage_kernel<real, 1>;
+    case 2: return (void*)bs_stage_kernel<real, 2>;
+    case 3: return (void*)bs_stage_kernel<real, 3>;
+    default: return (void*)bs_stage_kernel<real, 4>;
+  }
+}
+template <typename real>
+KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
+  FlowArgs<real> k;
+  memset(&k, 0, sizeof(k));
+  fill_constants(s, k);
+  BsArgs<real> a;
+  memset(&a, 0, sizeof(a));
+  a.phi = (const real*)s->phi(cur);
+  a.vel = (const real*)s->vel(cur);
+  a.aprev = stage == 3 ? (const real*)s->acc(0) : (const real*)s->acc(1);  // stage 4: a2
+  a.aout = (real*)s->acc(stage == 1 ? 0 : stage == 2 ? 1 : 2);
+  a.a1 = (const real*)s->acc(0);
+  a.a3 = (const real*)s->acc(2);
+  a.phi_out = (real*)s->phi(cur ^ 1);
+  a.vel_out = (real*)s->vel(cur ^ 1);
+  a.part_e = s->part(0); a.part_q = s->part(1); a.part_ke = s->part(2);
+  a.state = s->state();
+  a.Nx = s->Nx; a.Ny = s->Ny; a.nseg = s->L.nseg; a.plane = k.plane;
+  // stage fields: phi2 = R(phi + dt/2 v), phi3 = R((phi + dt/2 v) + dt^2/4 a1),
+  // phi4 = R((phi + dt v) + dt^2/2 a2)
+  a.alpha = stage == 4 ? k.dt : k.hdt;
+  a.beta = stage == 3 ? k.qdt2 : k.hdt2;
+  a.dt = k.dt; a.sdt2 = k.sdt2; a.sdt = k.sdt;
+  a.i12h = k.i12h; a.i12h2 = k.i12h2;
+  a.lap0 = k.lap0; a.lap1 = k.lap1; a.lap2 = k.lap2;
+  a.jA = k.jA; a.jB = k.jB;
+  a.bs_k2 = k.bs_k2; a.bs_mu2 = k.bs_mu2; a.bs_pot = k.bs_pot; a.bs_potN = k.bs_potN;
+  KernelNode n;
+  n.func = bs_func<real>(stage);
+  n.grid = dim3((s->Nx + BTX - 1) / BTX, (s->Ny + BTY - 1) / BTY, s->batch);
+  n.block = dim3(BBX, BBY, 1);
+  n.smem = sizeof(BsSmem<real>);
+  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  static const char* names[4] = {"bs_stage1_grad_energy_charge", "bs_stage2", "bs_stage3",
+                                 "bs_stage4_combine_project_ke"};
+  n.name = names[stage - 1];
+  return n;
+}
+KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
+  return s->dtype == SS_F64 ? make_bs_node<double>(s, stage, cur)
+                            : make_bs_node<float>(s, stage, cur);
 }
 
 // chunks per segment: minimise (waves of CTAs) x (chunks marched per CTA, warm-up included)
@@ -384,6 +458,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
   if (p->flags & ~SS_FLAG_NO_GRAPH) return SS_ERR_ARG;
+  if (theory == SS_THEORY_BABY_SKYRME && (p->integrator != SS_RK4 || p->dmi_d))
+    return SS_ERR_UNSUPPORTED;  // the baby-Skyrme kernels exist for the RK4 step only
   if (p->dmi_d)
     for (int i = 0; i < 6; ++i)
       if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;
@@ -402,7 +478,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return SS_ERR_WORKSPACE;
   ss_solver* s = new (std::nothrow) ss_solver();
   if (!s) return SS_ERR_ARG;
-  s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_CHIRAL_MAGNET ? 3 : 4;
+  s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_ABELIAN_HIGGS ? 4 : 3;
+  s->mu = p->mu; s->pot = p->potential; s->potN = p->potential_n;
   s->Nx = Nx; s->Ny = Ny; s->batch = p->batch; s->h = h;
   s->device = pa.device;
   s->dt = p->dt > 0.0 ? p->dt : 0.5 * h;
@@ -414,7 +491,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->log_cap = p->arrest_log_capacity > 0 ? p->arrest_log_capacity : 4096;
   s->flags = p->flags;
   s->integrator = p->integrator;
-  s->ktheory = theory;
+  s->ktheory = theory == SS_THEORY_BABY_SKYRME ? kBS : theory;
+  for (int i = 0; i < 6; ++i) s->dmi[i] = 0.0;
   if (theory == SS_THEORY_CHIRAL_MAGNET && p->dmi_d) {
     s->ktheory = kCMG;
     for (int i = 0; i < 6; ++i) s->dmi[i] = p->dmi_d[i];
@@ -439,7 +517,26 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);  // bb is a local
   if (!cuda_ok(e, "upload B_batch")) { delete s; return SS_ERR_CUDA; }
 
-  for (int kind = 0; kind < 3; ++kind) {
+  if (p->dtype == SS_F64) {
+    FlowArgs<double> k;
+    memset(&k, 0, sizeof(k));
+    fill_constants(s, k);
+    s->consts.assign((unsigned char*)&k, (unsigned char*)&k + sizeof(k));
+  } else {
+    FlowArgs<float> k;
+    memset(&k, 0, sizeof(k));
+    fill_constants(s, k);
+    s->consts.assign((unsigned char*)&k, (unsigned char*)&k + sizeof(k));
+  }
+  if (s->ktheory == kBS) {
+    for (int stage = 1; stage <= 4; ++stage) {
+      void* f = p->dtype == SS_F64 ? bs_func<double>(stage) : bs_func<float>(stage);
+      const size_t smem = p->dtype == SS_F64 ? sizeof(BsSmem<double>) : sizeof(BsSmem<float>);
+      e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+    }
+  }
+  for (int kind = 0; kind < 3 && s->ktheory != kBS; ++kind) {
     void* f = flow_func(s->ktheory, p->dtype, kind);
     const int smem = flow_smem(s->ktheory, p->dtype, kind);
     e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -455,7 +552,13 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
-    if (s->integrator == SS_VERLET) {
+    if (s->ktheory == kBS) {
+      st.push_back(make_bs_node(s, 2, cur));
+      st.push_back(make_bs_node(s, 3, cur));
+      st.push_back(make_bs_node(s, 4, cur));
+      st.push_back(make_bs_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
+      ev.push_back(make_bs_node(s, 1, cur));
+    } else if (s->integrator == SS_VERLET) {
       KernelNode v, x0;
       if (!make_flow_node(s, KV, cur, &v) || !make_flow_node(s, KX, cur, &x0)) {
         ss_destroy(s);
@@ -711,7 +814,7 @@ int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_ker
 
 template <int THEORY, typename real>
 static int render_t(ss_solver* s, int obs, int lattice, void* rgba_dev, double* minmax_host) {
-  const FlowArgs<real>& fa = *reinterpret_cast<const FlowArgs<real>*>(s->eval_nodes[0][0].args.data());
+  const FlowArgs<real>& fa = *reinterpret_cast<const FlowArgs<real>*>(s->consts.data());
   RenderArgs<real> r;
   memset(&r, 0, sizeof(r));
   const size_t sites = (size_t)s->Nx * s->Ny;
@@ -755,6 +858,8 @@ int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double*
                          : render_t<kCM, float>(s, observable, lattice, rgba_dev, minmax_host);
     case kAH: return f64 ? render_t<kAH, double>(s, observable, lattice, rgba_dev, minmax_host)
                          : render_t<kAH, float>(s, observable, lattice, rgba_dev, minmax_host);
+    case kBS: return f64 ? render_t<kBS, double>(s, observable, lattice, rgba_dev, minmax_host)
+                         : render_t<kBS, float>(s, observable, lattice, rgba_dev, minmax_host);
     default:  return f64 ? render_t<kCMG, double>(s, observable, lattice, rgba_dev, minmax_host)
                          : render_t<kCMG, float>(s, observable, lattice, rgba_dev, minmax_host);
   }

@@ -6,7 +6,8 @@
 
 namespace ss {
 
-constexpr int kCM = 0, kAH = 1, kCMG = 2;  // kCMG: chiral magnet with a general DMI table
+// kernel families: kCMG = chiral magnet with a general DMI table, kBS = baby Skyrme
+constexpr int kCM = 0, kAH = 1, kCMG = 2, kBS = 3;
 constexpr int HALO = 2;  // PAPER.md:102 "fourth-order ... stencils and halo width two"
 
 // Row segment of the canonical reduction tree (DESIGN R10): per-row partial sums are stored

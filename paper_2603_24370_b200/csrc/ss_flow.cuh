@@ -61,6 +61,8 @@ struct FlowArgs {
   real dm1, dm2, K2;              // 2 kappa (8, 1) / (12 h); 2 K
   real jA, jB, hk, qs;            // J1/4h^2, J2/4h^2, kappa/(12h), 1/(4 pi (12h)^2)
   real dk[6];                     // kappa/(12h) * (d_x, d_y)   (general DMI table)
+  real bs_k2, bs_mu2;             // baby Skyrme: kappa^2, mu^2
+  int bs_pot, bs_potN;            //              potential, N of the Z_N one
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {

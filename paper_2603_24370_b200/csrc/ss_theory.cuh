@@ -438,9 +438,115 @@ struct AH {
   __device__ __forceinline__ static void project_velocity(real*, const real*) {}
 };
 
+// ------------------------------------------------------------------ baby Skyrme
+// E = 1/2 |grad m|^2 + (kappa^2/2) |D_x m x D_y m|^2 + V(m), m in S^2 (PAPER.md:323 Table 2, :90;
+// DESIGN R18).  Dirichlet term as the chiral magnet's exchange (bond form, halo weights R3);
+// Skyrme term and potential are site sums over the interior with eq. (1).  Exact gradient in flux
+// form: a = D_x m, b = D_y m, w = a x b, F_x = kappa^2 (b x w), F_y = kappa^2 (w x a) (0 on the
+// halo), G = -(Lx + Ly) m - D_x F_x - D_y F_y + dV/dm -- radius 4, evaluated by the tile kernels
+// of ss_bs.cuh in two passes.  p supplies i12h, jA, jB, bs_k2 = kappa^2, bs_mu2, bs_pot, bs_potN.
+template <typename real>
+struct BS {
+  static constexpr int C = 3;
+  static constexpr int POT_STANDARD = 0, POT_EASY_PLANE = 1, POT_BROKEN = 2;
+
+  __device__ __forceinline__ static void cpow(real x, real y, int N, real& re, real& im) {
+    real a = real(1), b = real(0);
+    for (int k = 0; k < N; ++k) {
+      const real t = a * x - b * y;
+      b = a * y + b * x;
+      a = t;
+    }
+    re = a;
+    im = b;
+  }
+  // standard mu^2 (1 - m3); easy plane 1/2 mu^2 m1^2; broken mu^2 |1 - (m1 + i m2)^N|^2 (1 - m3)
+  template <typename P>
+  __device__ __forceinline__ static real potential(const P& p, real m1, real m2, real m3) {
+    if (p.bs_pot == POT_STANDARD) return p.bs_mu2 * (real(1) - m3);
+    if (p.bs_pot == POT_EASY_PLANE) return real(0.5) * p.bs_mu2 * (m1 * m1);
+    real a, b;
+    cpow(m1, m2, p.bs_potN, a, b);
+    return p.bs_mu2 * ((real(1) - a) * (real(1) - a) + b * b) * (real(1) - m3);
+  }
+  template <typename P>
+  __device__ __forceinline__ static void potential_grad(const P& p, real m1, real m2, real m3,
+                                                        real dV[3]) {
+    if (p.bs_pot == POT_STANDARD) { dV[0] = real(0); dV[1] = real(0); dV[2] = -p.bs_mu2; return; }
+    if (p.bs_pot == POT_EASY_PLANE) { dV[0] = p.bs_mu2 * m1; dV[1] = real(0); dV[2] = real(0); return; }
+    real a, b, c, d;
+    const real N = real(p.bs_potN);
+    cpow(m1, m2, p.bs_potN, a, b);
+    cpow(m1, m2, p.bs_potN - 1, c, d);
+    const real P2 = (real(1) - a) * (real(1) - a) + b * b;
+    dV[0] = p.bs_mu2 * (real(1) - m3) * (real(2) * N * (b * d - (real(1) - a) * c));
+    dV[1] = p.bs_mu2 * (real(1) - m3) * (real(2) * N * ((real(1) - a) * d + b * c));
+    dV[2] = -p.bs_mu2 * P2;
+  }
+  // a = D_x m, b = D_y m, w = a x b at the site
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void derivs(const Tile& T, const P& p, real a[3], real b[3],
+                                                real w[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      a[c] = p.i12h * Dxn<real>(T, c);
+      b[c] = p.i12h * Dyn<real>(T, c);
+    }
+    w[0] = a[1] * b[2] - a[2] * b[1];
+    w[1] = a[2] * b[0] - a[0] * b[2];
+    w[2] = a[0] * b[1] - a[1] * b[0];
+  }
+  template <typename P>
+  __device__ __forceinline__ static void flux(const P& p, const real a[3], const real b[3],
+                                              const real w[3], real Fx[3], real Fy[3]) {
+    Fx[0] = p.bs_k2 * (b[1] * w[2] - b[2] * w[1]);
+    Fx[1] = p.bs_k2 * (b[2] * w[0] - b[0] * w[2]);
+    Fx[2] = p.bs_k2 * (b[0] * w[1] - b[1] * w[0]);
+    Fy[0] = p.bs_k2 * (w[1] * a[2] - w[2] * a[1]);
+    Fy[1] = p.bs_k2 * (w[2] * a[0] - w[0] * a[2]);
+    Fy[2] = p.bs_k2 * (w[0] * a[1] - w[1] * a[0]);
+  }
+  // site-form energy density and degree density from w = D_x m x D_y m
+  template <typename Tile, typename P, typename W>
+  __device__ __forceinline__ static void densities_w(const Tile& T, const P& p, const W& wt,
+                                                     const real w[3], real& e, real& q) {
+    const real m[3] = {T(0, 0, 0), T(1, 0, 0), T(2, 0, 0)};
+    const int ks[4] = {1, -1, 2, -2};
+    real sA = real(0), sB = real(0);
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      real tx = real(0), ty = real(0);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const real ax = m[c] - T(c, 0, ks[s]), ay = m[c] - T(c, ks[s], 0);
+        tx += ax * ax;
+        ty += ay * ay;
+      }
+      const real t = real(wt.wx(s)) * tx + real(wt.wy(s)) * ty;
+      if (s < 2) sA += t; else sB += t;
+    }
+    e = (p.jA * sA + p.jB * sB) +
+        real(0.5) * p.bs_k2 * ((w[0] * w[0] + w[1] * w[1]) + w[2] * w[2]) +
+        potential(p, m[0], m[1], m[2]);
+    q = real(0.07957747154594767) * ((m[0] * w[0] + m[1] * w[1]) + m[2] * w[2]);
+  }
+  template <typename Tile, typename P, typename W>
+  __device__ __forceinline__ static void densities(const Tile& T, const P& p, real, const W& wt,
+                                                   real& e, real& q) {
+    real a[3], b[3], w[3];
+    derivs(T, p, a, b, w);
+    densities_w(T, p, wt, w, e, q);
+  }
+  __device__ __forceinline__ static void project_field(real m[3]) { CM<real>::project_field(m); }
+  __device__ __forceinline__ static void project_velocity(real u[3], const real n[3]) {
+    CM<real>::project_velocity(u, n);
+  }
+};
+
 template <int THEORY, typename real> struct TheoryOf;
 template <typename real> struct TheoryOf<kCM, real> { using type = CM<real>; };
 template <typename real> struct TheoryOf<kAH, real> { using type = AH<real>; };
 template <typename real> struct TheoryOf<kCMG, real> { using type = CMG<real>; };
+template <typename real> struct TheoryOf<kBS, real> { using type = BS<real>; };
 
 }  // namespace ss

@@ -19,7 +19,8 @@ if not os.path.exists(LIB_PATH):
         "(nvcc, sm_100a).  There is no CPU fallback.")
 _lib = C.CDLL(LIB_PATH)
 
-THEORY_CHIRAL_MAGNET, THEORY_ABELIAN_HIGGS = 0, 1
+THEORY_CHIRAL_MAGNET, THEORY_ABELIAN_HIGGS, THEORY_BABY_SKYRME = 0, 1, 2
+POT_STANDARD, POT_EASY_PLANE, POT_BROKEN = 0, 1, 2
 F64, F32 = 0, 1
 OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE = \
     0, -1, -2, -3, -4, -5, -6
@@ -40,7 +41,8 @@ class ss_params(C.Structure):
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("stream", C.c_void_p), ("arrest_log_capacity", C.c_int64),
                 ("integrator", C.c_int), ("flags", C.c_int),
-                ("chunks_per_segment", C.c_int), ("dmi_d", C.POINTER(C.c_double))]
+                ("chunks_per_segment", C.c_int), ("dmi_d", C.POINTER(C.c_double)),
+                ("mu", C.c_double), ("potential", C.c_int), ("potential_n", C.c_int)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -87,8 +89,9 @@ def _check(rc, where, allow=()):
 
 
 def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, integrator=0,
-            dmi=None):
+            dmi=None, mu=0.0, pot=0, potN=3):
     p = ss_params()
+    p.mu, p.potential, p.potential_n = float(mu), int(pot), int(potN)
     p.dtype, p.batch, p.dt = int(dtype), int(batch), float(dt)
     p.kappa, p.B, p.K, p.lam = float(kappa), float(B), float(K), float(lam)
     keep = None
@@ -116,16 +119,16 @@ class Solver:
 
     def __init__(self, theory, Nx, Ny, h, *, dtype=F64, batch=1, dt=0.0, kappa=0.0, B=0.0, K=0.0,
                  lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, integrator=RK4, dmi=None,
-                 device="cuda:0", stream=None):
+                 mu=0.0, pot=POT_STANDARD, potN=3, device="cuda:0", stream=None):
         self.theory, self.Nx, self.Ny, self.batch = int(theory), int(Nx), int(Ny), int(batch)
-        self.C = 3 if theory == THEORY_CHIRAL_MAGNET else 4
+        self.C = 4 if theory == THEORY_ABELIAN_HIGGS else 3
         self.dtype = dtype
         self.log_cap = int(log_cap) if log_cap else 4096
         self.torch_dtype = torch.float64 if dtype == F64 else torch.float32
         self.device = torch.device(device)
         self._h = C.c_void_p()
         p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps,
-                          integrator, dmi)
+                          integrator, dmi, mu, pot, potN)
         nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
         if nbytes == 0:
             # invalid or over a limit: ss_create tells which (it checks before touching memory)
@@ -271,4 +274,6 @@ def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0,
     """Solver configured from a workloads.Workload (sizes and parameters only)."""
     return Solver(w.theory, w.Nx, w.Ny, w.h, dtype=dtype, batch=w.batch, dt=w.dt, kappa=w.kappa,
                   B=w.B, K=w.K, lam=w.lam, B_batch=w.B_batch, log_cap=log_cap, flags=flags,
-                  cps=cps, integrator=integrator, dmi=getattr(w, "dmi", None), device=device)
+                  cps=cps, integrator=integrator, dmi=getattr(w, "dmi", None),
+                  mu=getattr(w, "mu", 0.0), pot=getattr(w, "pot", 0), potN=getattr(w, "potN", 3),
+                  device=device)

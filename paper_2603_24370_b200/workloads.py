@@ -212,6 +212,11 @@ def bs_single(N=128, h=0.2, kappa=1.0, mu=1.0, pot=POT_STANDARD, potN=3, noise=0
                     batch=batch, steps=steps, fields=f)
 
 
+def bs_bench() -> Workload:
+    """The baby-Skyrme bench workload: 2048^2, 32 hedgehogs, standard potential."""
+    return bs_single(N=2048, count=32, steps=2000)
+
+
 def baseline_config(c: int, **kw) -> Workload:
     """BASELINE.json configs[c-1] at full size (override sizes with kw for scaled copies)."""
     return {1: cm_single, 2: cm_multi, 3: ah_vortices, 4: cm_quench, 5: cm_sweep}[c](**kw)
