@@ -73,8 +73,10 @@ enum {
 enum { SS_RK4 = 0, SS_VERLET = 1 };
 
 /* ss_params.flags (debugging aid, not part of the method) */
-enum { SS_FLAG_NO_GRAPH = 1 }; /* launch the step's kernels one by one instead of replaying the
+enum { SS_FLAG_NO_GRAPH = 1,   /* launch the step's kernels one by one instead of replaying the
                                   per-step CUDA graphs; results are bitwise identical */
+       SS_FLAG_NO_RESIDENT = 2 /* never use the resident-cluster schedule (see ss_step); results
+                                  are bitwise identical */ };
 
 typedef struct {
   int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
@@ -92,7 +94,7 @@ typedef struct {
   int64_t arrest_log_capacity; /* entries per lattice; 0 -> 4096; later arrests are counted */
                                /* but not logged                                            */
   int integrator;          /* SS_RK4 | SS_VERLET                                            */
-  int flags;               /* 0 or SS_FLAG_NO_GRAPH                                         */
+  int flags;               /* 0 or a combination of SS_FLAG_*                                */
   int chunks_per_segment;  /* tuning, 0 = auto: rows/4 each CTA of the flow kernels marches */
                            /* (results do not depend on it)                                 */
   const double* dmi_d;     /* chiral magnet, optional HOST array[6] = (d_x, d_y): the DMI term   */
@@ -142,7 +144,11 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
 /* Enqueue k flow steps (asynchronous; no host synchronisation, the arrest of eq. 4 is
  * decided on the device; the steps are CUDA-graph replays, 8 steps per graph launch plus
  * single-step graphs for the remainder).  One step = RK4 stages 2-4 + update + projection, then the
- * stencil pass on the new field (a, E, Q) and the arrest decision. */
+ * stencil pass on the new field (a, E, Q) and the arrest decision.
+ * Small lattices (fp64 chiral magnet, SS_RK4, Nx a multiple of 32, the whole state within the
+ * shared memory of one thread-block cluster per lattice, e.g. 64 x 64 ... 128 x 128) take all k
+ * steps in ONE launch with the state resident in shared memory; fields, E, Q, KE and the arrest
+ * log are bitwise identical to the general schedule. */
 int ss_step(ss_solver* s, int64_t k);
 
 /* Scalar read-outs: synchronise the stream, then fill HOST arrays of length batch.
@@ -193,6 +199,8 @@ int64_t ss_launch_count(const ss_solver* s);
  * exactly as with ss_step(reps).  Synchronises the stream. */
 int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_kernels);
 const char* ss_kernel_name(const ss_solver* s, int i);
+/* Name of the schedule ss_step uses for this solver ("two-kernel", "resident-cluster", ...). */
+const char* ss_schedule_name(const ss_solver* s);
 
 #ifdef __cplusplus
 }

@@ -15,6 +15,7 @@
 #include "ss_flow.cuh"
 #include "ss_kernels.cuh"
 #include "ss_render.cuh"
+#include "ss_resident.cuh"
 
 using namespace ss;
 
@@ -133,6 +134,8 @@ struct ss_solver {
   cudaGraphExec_t step_exec[2];   // one flow step, per ping-pong parity
   cudaGraphExec_t multi_exec[2];  // MULTI consecutive steps in one graph (k steps per launch)
   std::vector<unsigned char> consts;  // FlowArgs<real> holding the per-site constants (ss_render)
+  int res_cl, res_rows;               // resident-cluster schedule: cluster size (0 = off), rows/CTA
+  size_t res_smem;
   std::vector<LatticeState> host_state;
   std::vector<double> Bb_host;  // per-lattice Zeeman field (host copy)
 
@@ -436,6 +439,76 @@ int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* e
   return SS_OK;
 }
 
+// Resident-cluster schedule (ss_resident.cuh): chiral magnet, default DMI, fp64, RK4, lattices
+// whose state fits in the shared memory of one cluster and whose clusters fit on the device at once
+void choose_resident(ss_solver* s) {
+  s->res_cl = 0;
+  if (s->ktheory != kCM || s->dtype != SS_F64 || s->integrator != SS_RK4) return;
+  if (s->flags & SS_FLAG_NO_RESIDENT) return;
+  if (s->Nx % 32 != 0 || s->Nx > 1024 || s->Ny > RES_MAX_NY) return;
+  const int order[5] = {16, 8, 4, 2, 1};  // most SMs first: the fp64 pipes bound the step
+  for (int i = 0; i < 5; ++i) {
+    const int cl = order[i];
+    if (s->Ny % cl != 0 || (cl > 1 && s->Ny / cl < 2 * HALO)) continue;
+    if ((long long)cl * s->batch > s->sms) continue;
+    const size_t smem = resident_smem_doubles(s->Nx, s->Ny, s->Ny / cl) * sizeof(double);
+    if (smem > 227 * 1024) continue;
+    if (cudaFuncSetAttribute((void*)resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)smem) != cudaSuccess ||
+        (cl > 8 && cudaFuncSetAttribute((void*)resident_kernel,
+                                        cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+      cudaGetLastError();
+      continue;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(cl, s->batch, 1);
+    cfg.blockDim = dim3(RES_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int nclusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclusters, (void*)resident_kernel, &cfg) != cudaSuccess ||
+        nclusters < s->batch) {
+      cudaGetLastError();
+      continue;
+    }
+    s->res_cl = cl; s->res_rows = s->Ny / cl; s->res_smem = smem;
+    return;
+  }
+}
+
+int resident_step(ss_solver* s, int64_t k) {
+  ResidentArgs a;
+  memset(&a, 0, sizeof(a));
+  a.k = *reinterpret_cast<const FlowArgs<double>*>(s->consts.data());
+  a.phi = (double*)s->phi(s->cur); a.vel = (double*)s->vel(s->cur);
+  a.a1 = (double*)s->acc(0); a.a2 = (double*)s->acc(1);
+  a.state = s->state();
+  a.log = (long long*)(s->ws + s->L.off_log);
+  a.log_cap = s->log_cap;
+  a.Bb = (const double*)(s->ws + s->L.off_bb);
+  a.rows = s->res_rows;
+  a.steps = k;
+  a.h2 = s->h * s->h;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(s->res_cl, s->batch, 1);
+  cfg.blockDim = dim3(RES_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = s->res_smem;
+  cfg.stream = s->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = s->res_cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  CK(cudaLaunchKernelEx(&cfg, resident_kernel, a));
+  s->launches += 1;
+  s->steps_done += k;
+  return SS_OK;
+}
+
 int read_state(ss_solver* s) {
   CK(cudaMemcpyAsync(s->host_state.data(), s->state(), s->batch * sizeof(LatticeState),
                      cudaMemcpyDeviceToHost, s->stream));
@@ -457,7 +530,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   *out = nullptr;
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
-  if (p->flags & ~SS_FLAG_NO_GRAPH) return SS_ERR_ARG;
+  if (p->flags & ~(SS_FLAG_NO_GRAPH | SS_FLAG_NO_RESIDENT)) return SS_ERR_ARG;
   if (theory == SS_THEORY_BABY_SKYRME && (p->integrator != SS_RK4 || p->dmi_d))
     return SS_ERR_UNSUPPORTED;  // the baby-Skyrme kernels exist for the RK4 step only
   if (p->dmi_d)
@@ -595,6 +668,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (rc != SS_OK) { ss_destroy(s); return rc; }
     }
   }
+  choose_resident(s);
   *out = s;
   return SS_OK;
 }
@@ -700,6 +774,7 @@ int ss_step(ss_solver* s, int64_t k) {
   if (!s || k < 0) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
   GUARD(s);
+  if (s->res_cl > 0 && k > 0) return resident_step(s, k);
   for (int64_t it = 0; it < k; ++it) {
     if (s->flags & SS_FLAG_NO_GRAPH) {
       int rc = launch_nodes(s, s->step_nodes[s->cur]);
@@ -863,6 +938,13 @@ int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double*
     default:  return f64 ? render_t<kCMG, double>(s, observable, lattice, rgba_dev, minmax_host)
                          : render_t<kCMG, float>(s, observable, lattice, rgba_dev, minmax_host);
   }
+}
+
+const char* ss_schedule_name(const ss_solver* s) {
+  if (!s) return "";
+  if (s->res_cl > 0) return "resident-cluster";
+  if (s->ktheory == kBS) return "per-stage tile kernels";
+  return s->integrator == SS_VERLET ? "one-kernel verlet" : "two-kernel";
 }
 
 const char* ss_kernel_name(const ss_solver* s, int i) {

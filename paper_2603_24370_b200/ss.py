@@ -27,11 +27,12 @@ OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE 
 RK4, VERLET = 0, 1
 OBS_ENERGY, OBS_CHARGE, OBS_ORDER = 0, 1, 2
 FLAG_NO_GRAPH = 1
+FLAG_NO_RESIDENT = 2
 
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
            "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",
            "ss_step", "ss_energy", "ss_charge", "ss_kinetic", "ss_status", "ss_arrests",
-           "ss_launch_count", "ss_strerror", "ss_render"]
+           "ss_launch_count", "ss_strerror", "ss_render", "ss_schedule_name"]
 
 
 class ss_params(C.Structure):
@@ -58,6 +59,8 @@ _lib.ss_get_fields_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ss_profile_step.argtypes = [C.c_void_p, C.c_int, _dp, C.c_int, C.POINTER(C.c_int)]
 _lib.ss_kernel_name.argtypes = [C.c_void_p, C.c_int]
 _lib.ss_kernel_name.restype = C.c_char_p
+_lib.ss_schedule_name.argtypes = [C.c_void_p]
+_lib.ss_schedule_name.restype = C.c_char_p
 _lib.ss_step.argtypes = [C.c_void_p, C.c_int64]
 for _n in ("ss_energy", "ss_charge", "ss_kinetic"):
     getattr(_lib, _n).argtypes = [C.c_void_p, _dp]
@@ -264,6 +267,9 @@ class Solver:
                    allow=() if strict else (ERR_NONFINITE,))
         self._before_current()
         return img, (mm[0], mm[1])
+
+    def schedule(self) -> str:
+        return _lib.ss_schedule_name(self._h).decode()
 
     def launch_count(self) -> int:
         return _lib.ss_launch_count(self._h)
