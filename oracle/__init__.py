@@ -35,7 +35,7 @@ class _Model(C.Structure):
     _fields_ = [("theory", C.c_int), ("Nx", C.c_int), ("Ny", C.c_int), ("h", C.c_double),
                 ("kappa", C.c_double), ("B", C.c_double), ("K", C.c_double),
                 ("lam", C.c_double), ("dmi", C.c_int), ("d", C.c_double * 6),
-                ("pot", C.c_int), ("potN", C.c_int), ("mu", C.c_double)]
+                ("pot", C.c_int), ("potN", C.c_int), ("mu", C.c_double), ("demag", C.c_double)]
 
 
 _lib = None
@@ -58,6 +58,11 @@ def lib():
         L.orc_ah_energy_bond.restype = C.c_double
         L.orc_bs_energy_plain.argtypes = [C.POINTER(_Model), _dp]
         L.orc_bs_energy_plain.restype = C.c_double
+        L.orc_poisson_solve.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_double]
+        L.orc_poisson_solve.restype = C.c_int
+        L.orc_demag_potential.argtypes = [C.POINTER(_Model), _dp, _dp]
+        L.orc_demag_energy_plain.argtypes = [C.POINTER(_Model), _dp]
+        L.orc_demag_energy_plain.restype = C.c_double
         L.orc_energy_charge.argtypes = [C.POINTER(_Model), _dp, C.c_int, _dp, _dp, _dp, _dp]
         L.orc_gradient.argtypes = [C.POINTER(_Model), _dp, _dp]
         L.orc_accel.argtypes = [C.POINTER(_Model), _dp, _dp]
@@ -97,7 +102,7 @@ def ncomp(theory: int) -> int:
 
 
 def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None, mu=0.0,
-          pot=POT_STANDARD, potN=3):
+          pot=POT_STANDARD, potN=3, demag=0.0):
     """dmi: None = kappa n.(curl n) (BASELINE), else the six numbers (d_x, d_y) of
     PAPER.md:196 eq. (5): e_DMI = kappa sum_mu d_mu . (n x d_mu n).
     Baby Skyrme (theory BS): kappa = Skyrme coupling, V proportional to mu^2,
@@ -105,6 +110,7 @@ def model(theory, Nx, Ny, h, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None, mu=0.0,
     m = _Model(int(theory), int(Nx), int(Ny), float(h), float(kappa), float(B), float(K),
                float(lam))
     m.pot, m.potN, m.mu = int(pot), int(potN), float(mu)
+    m.demag = float(demag)     # chiral magnet: g = mu0 Ms^2 of PAPER.md:196 eq. (5), (6); 0 = off
     if dmi is not None:
         m.dmi = 1
         m.d = (C.c_double * 6)(*[float(x) for x in np.asarray(dmi).reshape(6)])
@@ -130,16 +136,33 @@ def tree_sum2d(v):
     return lib().orc_tree_sum2d(_p(v), v.shape[1], v.shape[0])
 
 
+def poisson_solve(rho, h, guess=None):
+    """(Lx + Ly) psi = rho on the interior, psi = 0 on the halo (eq. 2; conjugate gradients)."""
+    rho = _f64(rho)
+    psi = np.zeros_like(rho) if guess is None else _f64(guess).copy()
+    lib().orc_poisson_solve(_p(rho), _p(psi), rho.shape[1], rho.shape[0], float(h))
+    return psi
+
+
+def demag_potential(m, f):
+    """psi with lap psi = D_x n1 + D_y n2 (eq. 6 in units phi = mu0 Ms psi)."""
+    f = _f64(f)
+    psi = np.empty((m.Ny, m.Nx))
+    lib().orc_demag_potential(C.byref(m), _p(f), _p(psi))
+    return psi
+
+
 def energy_bond(m, f):
     """Plain bond-sum definition of E_h (straight summation)."""
     f = _f64(f)
     if m.theory == BS:
         return lib().orc_bs_energy_plain(C.byref(m), _p(f))
     if m.theory == CM:
+        Ed = lib().orc_demag_energy_plain(C.byref(m), _p(f)) if m.demag != 0.0 else 0.0
         if m.dmi:
             d = np.array(list(m.d))
-            return lib().orc_cm_energy_bond_d(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K, _p(d))
-        return lib().orc_cm_energy_bond(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K)
+            return Ed + lib().orc_cm_energy_bond_d(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K, _p(d))
+        return Ed + lib().orc_cm_energy_bond(_p(f), m.Nx, m.Ny, m.h, m.kappa, m.B, m.K)
     return lib().orc_ah_energy_bond(_p(f), m.Nx, m.Ny, m.h, m.lam)
 
 

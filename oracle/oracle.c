@@ -464,10 +464,127 @@ typedef struct {
   double d[6];   /* d_x, d_y of PAPER.md:196 eq. (5) */
   int pot, potN; /* baby Skyrme: potential (ORC_POT_*), and N of the Z_N-symmetric one */
   double mu;     /* baby Skyrme: V is proportional to mu^2 */
+  double demag;  /* chiral magnet: g = mu0 Ms^2 of the magnetostatic term (0 = off), see below */
 } orc_model;
 
 static int ncomp(int theory) { return theory == ORC_AH ? 4 : 3; }
 static int unit_field(int theory) { return theory != ORC_AH; } /* |m| = 1 constraint */
+
+/* ------------------------------------------------------ demagnetisation (chiral magnet) */
+/* PAPER.md:196 eq. (5) last term and :199-203 eq. (6): E_d = (1/2 mu0) int |grad phi|^2 with
+ * -lap phi = -mu0 div(Ms n), "solved self-consistently alongside n".  With phi = mu0 Ms psi and
+ * g = mu0 Ms^2 (DESIGN R19):   lap psi = div n = d1 n1 + d2 n2 ,   E_d = (g/2) int |grad psi|^2 ,
+ * and, because psi depends linearly on n through a symmetric operator, dE_d/dn = g (d1 psi, d2 psi, 0).
+ * Discrete: rho = D_x n1 + D_y n2 on I (eq. 1);  (Lx + Ly) psi = rho on I, psi = 0 on the halo
+ * (eq. 2; the potential of a texture that has decayed before the wall);  E_d = (g/2) sum over bonds
+ * (>= 1 interior end) J_k (psi_i - psi_j)^2, the |grad|^2 form of DESIGN R1;  gradient
+ * G += g (D_x psi, D_y psi, 0) -- exact for the exact solution of the linear system, because then
+ * E_d = -(g/2) h^2 sum_I psi rho and psi = L^-1 rho with L symmetric on the zero-extended space.
+ * The solve: conjugate gradients on the symmetric positive definite -L to a relative residual of
+ * 1e-15 (plain textbook CG; pinned by inverting the pinned stencil operator). */
+static void neg_lap_zero_ext(const double* x, double* y, int Nx, int Ny, double h) {
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i)
+      y[(size_t)j * Nx + i] =
+          interior(Nx, Ny, i, j) ? -(Lx(x, Nx, j, i, h) + Ly(x, Nx, j, i, h)) : 0.0;
+}
+static double dot_plane(const double* a, const double* b, size_t n) { /* straight sum */
+  double s = 0.0;
+  for (size_t k = 0; k < n; ++k) s += a[k] * b[k];
+  return s;
+}
+/* Solve (Lx + Ly) psi = rho on I with psi = 0 on the halo; rho is read on I only.
+ * psi is also the starting guess (its halo is overwritten with 0).  Returns the iterations. */
+int orc_poisson_solve(const double* rho, double* psi, int Nx, int Ny, double h) {
+  const size_t P = (size_t)Nx * Ny;
+  double *r = (double*)malloc(P * sizeof(double)), *p = (double*)malloc(P * sizeof(double)),
+         *q = (double*)malloc(P * sizeof(double));
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i)
+      if (!interior(Nx, Ny, i, j)) psi[(size_t)j * Nx + i] = 0.0;
+  neg_lap_zero_ext(psi, q, Nx, Ny, h); /* r = b - A x with A = -L, b = -rho */
+  double bb = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i) {
+      size_t a = (size_t)j * Nx + i;
+      double b = interior(Nx, Ny, i, j) ? -rho[a] : 0.0;
+      r[a] = b - q[a];
+      p[a] = r[a];
+      bb += b * b;
+    }
+  double rr = dot_plane(r, r, P);
+  int it = 0;
+  const int maxit = 20 * (Nx + Ny) + 200;
+  while (it < maxit && rr > 1e-30 * bb && rr > 0.0) {
+    neg_lap_zero_ext(p, q, Nx, Ny, h);
+    double alpha = rr / dot_plane(p, q, P);
+    for (size_t k = 0; k < P; ++k) {
+      psi[k] += alpha * p[k];
+      r[k] -= alpha * q[k];
+    }
+    double rr2 = dot_plane(r, r, P);
+    double beta = rr2 / rr;
+    for (size_t k = 0; k < P; ++k) p[k] = r[k] + beta * p[k];
+    rr = rr2;
+    ++it;
+  }
+  free(r); free(p); free(q);
+  return it;
+}
+/* psi of a magnetisation field n ([3][Ny][Nx]); psi [Ny][Nx], halo 0 */
+void orc_demag_potential(const orc_model* m, const double* n, double* psi) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  const size_t P = (size_t)Nx * Ny;
+  double* rho = (double*)calloc(P, sizeof(double));
+  for (int j = 2; j < Ny - 2; ++j)
+    for (int i = 2; i < Nx - 2; ++i)
+      rho[(size_t)j * Nx + i] = Dx(n, Nx, j, i, m->h) + Dy(n + P, Nx, j, i, m->h);
+  memset(psi, 0, P * sizeof(double));
+  orc_poisson_solve(rho, psi, Nx, Ny, m->h);
+  free(rho);
+}
+/* plain definition of E_d: bond loop, straight summation */
+static double demag_energy_bond(const orc_model* m, const double* psi) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  double E = 0.0;
+  for (int j = 0; j < Ny; ++j)
+    for (int i = 0; i < Nx; ++i)
+      for (int mu = 0; mu < 2; ++mu)
+        for (int k = 1; k <= 2; ++k) {
+          int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+          if (!inside(Nx, Ny, i2, j2)) continue;
+          if (!interior(Nx, Ny, i, j) && !interior(Nx, Ny, i2, j2)) continue;
+          double d = psi[(size_t)j * Nx + i] - psi[(size_t)j2 * Nx + i2];
+          E += 0.5 * m->demag * Jw[k] * (d * d);
+        }
+  return E;
+}
+/* site form (DESIGN R3): e_d,i = g sum_mu sum_k w(j) J_|k|/(4 h^2) (psi_i - psi_j)^2, i in I;
+ * h^2 sum_I e_d,i equals the bond sum (each interior-interior bond is seen from both ends) */
+static double demag_site_energy(const orc_model* m, const double* psi, int j, int i) {
+  const int Nx = m->Nx, Ny = m->Ny;
+  static const int ks[4] = {1, -1, 2, -2};
+  double e = 0.0;
+  for (int mu = 0; mu < 2; ++mu)
+    for (int q = 0; q < 4; ++q) {
+      int k = ks[q], ak = k < 0 ? -k : k;
+      int i2 = i + (mu == 0 ? k : 0), j2 = j + (mu == 1 ? k : 0);
+      double w = interior(Nx, Ny, i2, j2) ? 1.0 : 2.0;
+      double d = psi[(size_t)j * Nx + i] - psi[(size_t)j2 * Nx + i2];
+      e += w * (Jw[ak] / (4.0 * (m->h * m->h)) * (d * d));
+    }
+  return m->demag * e;
+}
+
+/* plain E_d for the pins: (g/2) sum_bonds J_k (psi_i - psi_j)^2 of the solved potential */
+double orc_demag_energy_plain(const orc_model* m, const double* n) {
+  double* psi = (double*)malloc((size_t)m->Nx * m->Ny * sizeof(double));
+  orc_demag_potential(m, n, psi);
+  double E = demag_energy_bond(m, psi);
+  free(psi);
+  return E;
+}
 
 /* ------------------------------------------------------------------ baby Skyrme */
 /* Functional (Table 2; model list PAPER.md:90):
@@ -626,6 +743,11 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
   size_t P = (size_t)Nx * Ny;
   double* e = dens_e ? dens_e : (double*)malloc(P * sizeof(double));
   double* q = dens_q ? dens_q : (double*)malloc(P * sizeof(double));
+  double* psi = NULL;
+  if (m->theory == ORC_CM && m->demag != 0.0) {
+    psi = (double*)malloc(P * sizeof(double));
+    orc_demag_potential(m, f, psi);
+  }
 #pragma omp parallel for schedule(static)
   for (int j = 0; j < Ny; ++j)
     for (int i = 0; i < Nx; ++i) {
@@ -637,6 +759,7 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
         e[a] = m->dmi ? cm_site_energy_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d)
                       : cm_site_energy(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K);
         q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h);
+        if (psi) e[a] = e[a] + demag_site_energy(m, psi, j, i);
       } else if (m->theory == ORC_BS) {
         e[a] = bs_site_energy(m, f, j, i);
         q[a] = cm_site_charge(f, Nx, Ny, j, i, m->h); /* the same degree density */
@@ -648,6 +771,7 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
     }
   *E = (m->h * m->h) * orc_tree_sum2d(e, Nx, Ny);
   *Q = (m->h * m->h) * orc_tree_sum2d(q, Nx, Ny);
+  free(psi);
   if (!dens_e) free(e);
   if (!dens_q) free(q);
 }
@@ -655,7 +779,11 @@ void orc_energy_charge(const orc_model* m, const double* f, int which_energy, do
 /* Raw gradient G on the interior (halo entries 0), [C][Ny][Nx]. */
 void orc_gradient(const orc_model* m, const double* f, double* G) {
   const int Nx = m->Nx, Ny = m->Ny, C = ncomp(m->theory);
-  double *Fx = NULL, *Fy = NULL;
+  double *Fx = NULL, *Fy = NULL, *psi = NULL;
+  if (m->theory == ORC_CM && m->demag != 0.0) {
+    psi = (double*)malloc((size_t)Nx * Ny * sizeof(double));
+    orc_demag_potential(m, f, psi);
+  }
   if (m->theory == ORC_BS) {
     Fx = (double*)malloc(3 * (size_t)Nx * Ny * sizeof(double));
     Fy = (double*)malloc(3 * (size_t)Nx * Ny * sizeof(double));
@@ -669,6 +797,10 @@ void orc_gradient(const orc_model* m, const double* f, double* G) {
         if (m->theory == ORC_CM) {
           if (m->dmi) cm_site_gradient_d(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, m->d, g);
           else cm_site_gradient(f, Nx, Ny, j, i, m->h, m->kappa, m->B, m->K, g);
+          if (psi) { /* + g grad_h psi (in-plane components) */
+            g[0] = g[0] + m->demag * Dx(psi, Nx, j, i, m->h);
+            g[1] = g[1] + m->demag * Dy(psi, Nx, j, i, m->h);
+          }
         } else if (m->theory == ORC_BS) {
           bs_site_gradient(m, f, Fx, Fy, j, i, g);
         } else {
@@ -679,6 +811,7 @@ void orc_gradient(const orc_model* m, const double* f, double* G) {
     }
   free(Fx);
   free(Fy);
+  free(psi);
 }
 
 /* Acceleration a = -Pi_f(G(f)) on the interior (eq. (3) with the tangent
