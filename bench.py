@@ -46,6 +46,7 @@ WORKLOADS = {
     "sweep256_f64": ("cm_sweep", {}, "f64"),           # BASELINE configs[4], 256 lattices
     "cm64_f64": ("cm_single", {}, "f64"),              # BASELINE configs[0] (launch-bound)
     "bs2048_f64": ("bs_bench", {}, "f64"),             # baby Skyrme (SURVEY 8(f) NEXT-2b)
+    "demag2048_f64": ("cm_demag_bench", {}, "f64"),    # demagnetisation (NEXT-4): --integrator verlet
 }
 
 
@@ -236,6 +237,11 @@ KERNEL_UNITS = {
     "bs_stage3": 4,                       # reads phi, v, a1         -> writes a3
     "bs_stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
     "bs_stage1_grad_energy_charge": 2,    # reads phi'               -> writes a1 (+ E, Q partials)
+    # demagnetisation (csrc/ss_demag.cuh), units of C*R with C = 3: drift reads phi, v, a, writes
+    # phi', w; kick reads phi', w, psi, writes a', v'; rho and the multigrid kernels move single
+    # planes and are reported by their time only
+    "demag_drift": 5,
+    "demag_kick_energy_charge_ke": 13.0 / 3.0,
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
@@ -274,6 +280,24 @@ def ncu_traffic(workload_key, integrator, kernel):
         except Exception:
             continue
     return None
+
+
+DEMAG_DEFAULT_CYCLES = 12                       # include/ss.h: demag_cycles = 0
+
+
+def mg_alg_bytes(w, cycles):
+    """Algorithmic bytes per step of the multigrid kernels (csrc/ss_demag.cuh header): per
+    V-cycle and level 4 sweeps x (read psi, rhs; write psi), one residual + restriction (read psi,
+    rhs; write 1/4 rhs, 1/4 psi), one prolongation (read psi, 1/4 coarse; write psi), fp64."""
+    nx, ny, sizes = w.Nx - 4, w.Ny - 4, []
+    while True:
+        sizes.append(nx * ny)
+        if (nx <= 8 and ny <= 8) or nx // 2 < 2 or ny // 2 < 2:
+            break
+        nx, ny = nx // 2, ny // 2
+    fine = sum(sizes[:-1]) * w.batch
+    return {"mg_smooth": cycles * 4 * 24 * fine, "mg_residual_restrict": cycles * 20 * fine,
+            "mg_prolong_add": cycles * 18 * fine, "demag_rho": 24 * sizes[0] * w.batch}
 
 
 def max_over_ranks(values, dist=None, device="cpu"):
@@ -365,15 +389,21 @@ def run_ours(args):
     peak, peak_src = peaks()
     C = w.C
     kern = {}
-    for name, kms in prof:
+    agg = {}
+    for name, kms in prof:                      # a kernel launched several times per step: summed
+        t = agg.setdefault(name, [0.0, 0])
+        t[0] += kms
+        t[1] += 1
+    mg = mg_alg_bytes(w, DEMAG_DEFAULT_CYCLES) if getattr(w, "demag", 0.0) else {}
+    for name, (kms, cnt) in agg.items():
         u = KERNEL_UNITS.get(name)
-        kern[name] = {"ms": kms}
-        if u:
-            kern[name]["alg_bytes"] = u * C * R * sites
-            kern[name]["gbs"] = u * C * R * sites / (kms * 1e-3) / 1e9
+        kern[name] = {"ms": kms, "launches_per_step": cnt}
+        if u or name in mg:
+            kern[name]["alg_bytes"] = mg[name] if name in mg else u * C * R * sites
+            kern[name]["gbs"] = kern[name]["alg_bytes"] / (kms * 1e-3) / 1e9
     dom = max((n for n in kern if "gbs" in kern[n]), key=lambda n: kern[n]["ms"])
     tot = sum(k["ms"] for k in kern.values())
-    units = sum(KERNEL_UNITS.get(n, 0) for n in kern)      # 10 (RK4: Y + X) or 6 (Verlet)
+    units = sum(kern[n].get("alg_bytes", 0) for n in kern) / (C * R * sites)  # 10 (RK4), 6 (Verlet)
     for n in kern:
         if "gbs" in kern[n]:
             kern[n]["frac"] = kern[n]["gbs"] / peak
@@ -390,7 +420,7 @@ def run_ours(args):
         "traffic": tr["bytes"] if tr else None, "traffic_source": tr["source"] if tr else None,
         "peak_source": peak_src, "kernel_ms": kern[dom]["ms"],
         "kernel_share_of_step": kern[dom]["ms"] / tot,
-        "alg_bytes_per_site": KERNEL_UNITS[dom] * C * R,
+        "alg_bytes_per_site": kern[dom]["alg_bytes"] / sites,
         "step": {
             "ms_graph": ms / args.steps,
             "ms_sum_of_kernels": tot,
@@ -476,7 +506,8 @@ def main():
         "config": {"workload": w.name, "theory": THEORY_NAME[w.theory], "Nx": w.Nx, "Ny": w.Ny, "batch": w.batch, "h": w.h,
                    "dt": w.dt, "kappa": w.kappa, "B": w.B, "K": w.K, "lambda": w.lam,
                    "integrator": args.integrator,
-                   "schedule": "per-stage tile kernels" if w.theory == 2 else "two-kernel",
+                   "schedule": r["s"].schedule(),
+                   "demag": getattr(w, "demag", 0.0),
                    "parallelism": f"replicas x{r['world']}",
                    "l2_policy": "working set (6 field arrays) larger than L2; no flush needed"
                    if 6 * r["field_bytes"] > 3 * 126e6 else

@@ -103,6 +103,12 @@ typedef struct {
   double mu;               /* baby Skyrme: V is proportional to mu^2 (kappa = Skyrme coupling)   */
   int potential;           /* baby Skyrme: SS_POT_*                                              */
   int potential_n;         /* baby Skyrme: N of SS_POT_BROKEN                                    */
+  double demag;            /* chiral magnet: g = mu0 Ms^2 >= 0 of the magnetostatic energy           */
+                           /* (g/2)|grad psi|^2, lap psi = d1 n1 + d2 n2, psi = 0 on the halo         */
+                           /* (PAPER.md:196 eq. 5, :199-203 eq. 6; DESIGN R19); 0 = off.  Needs       */
+                           /* SS_VERLET and SS_F64; psi is solved by multigrid V-cycles on the device */
+  int demag_cycles;        /* V-cycles per step, warm-started (0 -> 12; 4x as many in ss_set_fields); */
+                           /* contraction per cycle 0.27 (even sizes on every level) ... 0.65        */
 } ss_params;
 
 /* Limits of this build: 5 <= Nx <= 65536, 5 <= Ny <= 32768 (the device-side reduction tree of

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "ss_bs.cuh"
+#include "ss_demag.cuh"
 #include "ss_flow.cuh"
 #include "ss_kernels.cuh"
 #include "ss_render.cuh"
@@ -37,6 +38,12 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 constexpr int MULTI = 8;  // steps per multi-step graph (even)
 
+struct MgHostLevel {
+  size_t off_psi, off_tmp, off_rhs;  // [batch][ny+4][nx+4] fp64 each
+  int nx, ny;
+  double c;                          // 1 / (12 h_l^2)
+};
+
 struct Layout {
   size_t field_bytes;  // one [batch][C][Ny][Nx] array
   size_t part_bytes;   // one [batch][Ny][nseg] fp64 array
@@ -45,6 +52,8 @@ struct Layout {
   int nacc;            // acceleration arrays: a1, a2 (+ a3 for the baby-Skyrme stage kernels)
   size_t off_phi[2], off_vel[2], off_a[3], off_part[3], off_rows, off_state, off_log, off_bb;
   size_t off_render;   // ss_render scratch: block extrema of one lattice, extrema, flag
+  std::vector<MgHostLevel> mg;  // demagnetisation: multigrid hierarchy (level 0 = the lattice)
+  size_t off_mg, mg_bytes;
   size_t total;
   int nseg;
 };
@@ -97,6 +106,23 @@ Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
   L.off_log = o; o += L.log_bytes;
   L.off_bb = o; o += L.bb_bytes;
   L.off_render = o; o += L.render_bytes;
+  L.off_mg = o; L.mg_bytes = 0;
+  if (theory == SS_THEORY_CHIRAL_MAGNET && p->demag != 0.0) {
+    int nx = Nx - 4, ny = Ny - 4;
+    for (int l = 0;; ++l) {
+      MgHostLevel lv;
+      const size_t bytes = align_up((size_t)p->batch * (ny + 4) * (nx + 4) * sizeof(double));
+      lv.nx = nx; lv.ny = ny;
+      lv.c = 0.0;  // filled by ss_create (needs h)
+      lv.off_psi = o; o += bytes;
+      lv.off_tmp = o; o += bytes;
+      lv.off_rhs = o; o += bytes;
+      L.mg.push_back(lv);
+      if ((nx <= MG_COARSE_MAX && ny <= MG_COARSE_MAX) || nx / 2 < 2 || ny / 2 < 2) break;
+      nx /= 2; ny /= 2;
+    }
+    L.mg_bytes = o - L.off_mg;
+  }
   L.total = o;
   return L;
 }
@@ -114,7 +140,8 @@ struct KernelNode {
 struct ss_solver {
   int theory, dtype, C, Nx, Ny, batch;
   int device, sms;  // the device the workspace lives on (current at ss_create) and its SM count
-  double h, dt, kappa, B, K, lambda, mu;
+  double h, dt, kappa, B, K, lambda, mu, demag;
+  int demag_cycles;
   int pot, potN;
   size_t R;
   cudaStream_t stream;
@@ -362,6 +389,102 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
                             : make_bs_node<float>(s, stage, cur);
 }
 
+// ---- demagnetisation (ss_demag.cuh): nodes of n V-cycles and of the Verlet step around them
+KernelNode mg_node(void* func, const MgArgs& m, dim3 grid, dim3 block, size_t smem, const char* name) {
+  KernelNode n;
+  n.func = func; n.grid = grid; n.block = block; n.smem = smem; n.name = name;
+  n.args.assign((const unsigned char*)&m, (const unsigned char*)&m + sizeof(m));
+  return n;
+}
+void add_vcycle(const ss_solver* s, size_t l, std::vector<KernelNode>& out) {
+  const MgHostLevel& f = s->L.mg[l];
+  double* psi = (double*)(s->ws + f.off_psi);
+  double* tmp = (double*)(s->ws + f.off_tmp);
+  const double* rhs = (const double*)(s->ws + f.off_rhs);
+  const dim3 block(MGX, MGY, 1);
+  const dim3 grid((f.nx + MGX - 1) / MGX, (f.ny + MGY - 1) / MGY, s->batch);
+  MgArgs m;
+  memset(&m, 0, sizeof(m));
+  m.nx = f.nx; m.ny = f.ny; m.c = f.c; m.rhs = rhs;
+  {  // wall factor alpha_l = (1 - d_l)/d_l, d_l = 1/2 + 1/2^(l+1); 0 on the lattice itself
+    const double d = 0.5 + 0.5 / double(1 << l);
+    m.alpha = l == 0 ? 0.0 : (1.0 - d) / d;
+  }
+  if (l + 1 == s->L.mg.size()) {
+    m.out = psi;
+    out.push_back(mg_node((void*)mg_coarse_kernel, m, dim3(s->batch, 1, 1), dim3(1024, 1, 1),
+                          (size_t)3 * (f.nx + 4) * (f.ny + 4) * sizeof(double), "mg_coarse"));
+    return;
+  }
+  auto smooth2 = [&]() {  // two sweeps: psi -> tmp -> psi
+    MgArgs a = m;
+    a.in = psi; a.out = tmp;
+    out.push_back(mg_node((void*)mg_smooth_kernel, a, grid, block, 0, "mg_smooth"));
+    a.in = tmp; a.out = psi;
+    out.push_back(mg_node((void*)mg_smooth_kernel, a, grid, block, 0, "mg_smooth"));
+  };
+  smooth2();
+  const MgHostLevel& c = s->L.mg[l + 1];
+  const dim3 cgrid((c.nx + MGX - 1) / MGX, (c.ny + MGY - 1) / MGY, s->batch);
+  MgArgs r = m;
+  r.in = psi; r.out = (double*)(s->ws + c.off_rhs); r.out2 = (double*)(s->ws + c.off_psi);
+  r.cnx = c.nx; r.cny = c.ny;
+  out.push_back(mg_node((void*)mg_restrict_kernel, r, cgrid, block, 0, "mg_residual_restrict"));
+  add_vcycle(s, l + 1, out);
+  MgArgs pr = m;
+  pr.out = psi; pr.in = (const double*)(s->ws + c.off_psi); pr.cnx = c.nx; pr.cny = c.ny;
+  out.push_back(mg_node((void*)mg_prolong_kernel, pr, grid, block, 0, "mg_prolong_add"));
+  smooth2();
+}
+// step: drift(cur -> cur^1), rho, V-cycles, kick; evaluation (ss_set_fields): rho, 4x the V-cycles
+// from psi = 0, kick without the velocity update
+void make_demag_step(const ss_solver* s, int cur, std::vector<KernelNode>& st,
+                     std::vector<KernelNode>& ev) {
+  DemagStepArgs a;
+  memset(&a, 0, sizeof(a));
+  a.p = *reinterpret_cast<const FlowArgs<double>*>(s->consts.data());
+  const MgHostLevel& l0 = s->L.mg[0];
+  a.d.rho = (double*)(s->ws + l0.off_rhs);
+  a.d.psi = (const double*)(s->ws + l0.off_psi);
+  a.d.part_e = s->part(0); a.d.part_q = s->part(1); a.d.part_ke = s->part(2);
+  a.d.state = s->state();
+  a.d.Bb = (const double*)(s->ws + s->L.off_bb);
+  a.d.g = s->demag;
+  const long long plane = (long long)s->Nx * s->Ny;
+  const dim3 pgrid((unsigned)((plane + 255) / 256), 1, s->batch);
+  const dim3 kgrid((s->Nx + DTX - 1) / DTX, (s->Ny + DTY - 1) / DTY, s->batch);
+  void* kick = s->ktheory == kCMG ? (void*)demag_kick_kernel<kCMG> : (void*)demag_kick_kernel<kCM>;
+  auto node = [&](void* f, const DemagStepArgs& x, dim3 grid, dim3 block, const char* name) {
+    KernelNode n;
+    n.func = f; n.grid = grid; n.block = block; n.smem = 0; n.name = name;
+    n.args.assign((const unsigned char*)&x, (const unsigned char*)&x + sizeof(x));
+    return n;
+  };
+  {  // one step
+    DemagStepArgs x = a;
+    x.d.phi = (const double*)s->phi(cur); x.d.vel = (const double*)s->vel(cur);
+    x.d.acc = (const double*)s->acc(cur);
+    x.d.phi_out = (double*)s->phi(cur ^ 1); x.d.vel_out = (double*)s->vel(cur ^ 1);
+    st.push_back(node((void*)demag_drift_kernel, x, pgrid, dim3(256, 1, 1), "demag_drift"));
+    x.d.phi = (const double*)s->phi(cur ^ 1);
+    st.push_back(node((void*)demag_rho_kernel, x, pgrid, dim3(256, 1, 1), "demag_rho"));
+    for (int c = 0; c < s->demag_cycles; ++c) add_vcycle(s, 0, st);
+    x.d.vel = (const double*)s->vel(cur ^ 1); x.d.vel_out = (double*)s->vel(cur ^ 1);
+    x.d.acc_out = (double*)s->acc(cur ^ 1);
+    x.d.advance = 1;
+    st.push_back(node(kick, x, kgrid, dim3(DBX, DBY, 1), "demag_kick_energy_charge_ke"));
+  }
+  {  // evaluation of the state in buffer cur (only used with cur == 0)
+    DemagStepArgs x = a;
+    x.d.phi = (const double*)s->phi(cur);
+    ev.push_back(node((void*)demag_rho_kernel, x, pgrid, dim3(256, 1, 1), "demag_rho"));
+    for (int c = 0; c < 4 * s->demag_cycles; ++c) add_vcycle(s, 0, ev);
+    x.d.acc_out = (double*)s->acc(cur);
+    x.d.advance = 0;
+    ev.push_back(node(kick, x, kgrid, dim3(DBX, DBY, 1), "demag_kick_energy_charge_ke"));
+  }
+}
+
 // chunks per segment: minimise (waves of CTAs) x (chunks marched per CTA, warm-up included)
 int choose_cps(int nstrips, int Ny, int batch, int slots) {
   const int NC = (Ny + FR - 1) / FR;
@@ -533,6 +656,10 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (p->flags & ~(SS_FLAG_NO_GRAPH | SS_FLAG_NO_RESIDENT)) return SS_ERR_ARG;
   if (theory == SS_THEORY_BABY_SKYRME && (p->integrator != SS_RK4 || p->dmi_d))
     return SS_ERR_UNSUPPORTED;  // the baby-Skyrme kernels exist for the RK4 step only
+  if (!std::isfinite(p->demag) || p->demag < 0.0 || p->demag_cycles < 0) return SS_ERR_ARG;
+  if (p->demag != 0.0 && theory == SS_THEORY_CHIRAL_MAGNET &&
+      (p->integrator != SS_VERLET || p->dtype != SS_F64))
+    return SS_ERR_UNSUPPORTED;  // demagnetisation: fp64, one-gradient-per-step integrator only
   if (p->dmi_d)
     for (int i = 0; i < 6; ++i)
       if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;
@@ -553,6 +680,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (!s) return SS_ERR_ARG;
   s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_ABELIAN_HIGGS ? 4 : 3;
   s->mu = p->mu; s->pot = p->potential; s->potN = p->potential_n;
+  s->demag = theory == SS_THEORY_CHIRAL_MAGNET ? p->demag : 0.0;
+  s->demag_cycles = p->demag_cycles > 0 ? p->demag_cycles : 12;
   s->Nx = Nx; s->Ny = Ny; s->batch = p->batch; s->h = h;
   s->device = pa.device;
   s->dt = p->dt > 0.0 ? p->dt : 0.5 * h;
@@ -561,6 +690,17 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->stream = (cudaStream_t)p->stream;
   s->ws = (char*)p->workspace;
   s->L = L;
+  for (size_t l = 0; l < s->L.mg.size(); ++l) {
+    const double hl = h * double(1 << l);
+    s->L.mg[l].c = 1.0 / (12.0 * hl * hl);
+  }
+  if (s->demag != 0.0) {  // the coarsest level is relaxed by one CTA in shared memory
+    const MgHostLevel& lv = s->L.mg.back();
+    if ((size_t)3 * (lv.nx + 4) * (lv.ny + 4) * sizeof(double) > 200 * 1024) {
+      delete s;
+      return SS_ERR_UNSUPPORTED;  // very anisotropic lattice: no semi-coarsening in this build
+    }
+  }
   s->log_cap = p->arrest_log_capacity > 0 ? p->arrest_log_capacity : 4096;
   s->flags = p->flags;
   s->integrator = p->integrator;
@@ -601,6 +741,11 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     fill_constants(s, k);
     s->consts.assign((unsigned char*)&k, (unsigned char*)&k + sizeof(k));
   }
+  if (s->demag != 0.0) {
+    e = cudaFuncSetAttribute((void*)mg_coarse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             200 * 1024);
+    if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
+  }
   if (s->ktheory == kBS) {
     for (int stage = 1; stage <= 4; ++stage) {
       void* f = p->dtype == SS_F64 ? bs_func<double>(stage) : bs_func<float>(stage);
@@ -625,7 +770,9 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
-    if (s->ktheory == kBS) {
+    if (s->demag != 0.0) {
+      make_demag_step(s, cur, st, ev);
+    } else if (s->ktheory == kBS) {
       st.push_back(make_bs_node(s, 2, cur));
       st.push_back(make_bs_node(s, 3, cur));
       st.push_back(make_bs_node(s, 4, cur));
@@ -718,6 +865,7 @@ static int set_fields_impl(ss_solver* s, const void* fields, const void* vel, cu
   else
     init_halo_kernel<float><<<grid, 256, 0, s->stream>>>((float*)s->phi(1), (float*)s->vel(1),
                                                          (const float*)s->phi(0), s->Nx, s->Ny, planes);
+  if (s->L.mg_bytes) CK(cudaMemsetAsync(s->ws + s->L.off_mg, 0, s->L.mg_bytes, s->stream));
   // KE partials are only written by a step: 0 after ss_set_fields
   for (int i = 0; i < 3; ++i) CK(cudaMemsetAsync(s->part(i), 0, s->L.part_bytes, s->stream));
   init_state_kernel<<<(s->batch + 127) / 128, 128, 0, s->stream>>>(s->state(), s->batch);

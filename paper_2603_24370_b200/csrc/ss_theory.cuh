@@ -93,6 +93,23 @@ struct CM {
     a[2] = gn * n3 - G[2];
   }
 
+  // the raw gradient G of accel() (for callers that add further forces before the projection:
+  // the demagnetising field, ss_demag.cuh)
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void gradient(const Tile& T, const P& p, real B, real G[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const real s1 = (T(c, 0, 1) + T(c, 0, -1)) + (T(c, 1, 0) + T(c, -1, 0));
+      const real s2 = (T(c, 0, 2) + T(c, 0, -2)) + (T(c, 2, 0) + T(c, -2, 0));
+      G[c] = p.lap2 * s2 + (p.lap0 * T(c, 0, 0) - p.lap1 * s1);
+    }
+    G[0] += p.dm1 * (T(2, 1, 0) - T(2, -1, 0)) - p.dm2 * (T(2, 2, 0) - T(2, -2, 0));
+    G[1] -= p.dm1 * (T(2, 0, 1) - T(2, 0, -1)) - p.dm2 * (T(2, 0, 2) - T(2, 0, -2));
+    G[2] += p.dm1 * ((T(1, 0, 1) - T(1, 0, -1)) - (T(0, 1, 0) - T(0, -1, 0))) -
+            p.dm2 * ((T(1, 0, 2) - T(1, 0, -2)) - (T(0, 2, 0) - T(0, -2, 0)));
+    G[2] -= B + p.K2 * T(2, 0, 0);
+  }
+
   // accel + site-form energy density + charge density of a site whose neighbours are all
   // interior (weights 1): the eq. (1) numerators d_x n, d_y n are formed once and serve the DMI
   // force, the DMI energy kappa n.(curl_h n) and the charge; the exchange energy keeps the
@@ -232,6 +249,25 @@ struct CMG {
     real dx[3], dy[3];
     numerators(T, BulkW(), dx, dy);
     accel_from(T, p, B, dx, dy, a);
+  }
+  // the raw gradient G of accel()
+  template <typename Tile, typename P>
+  __device__ __forceinline__ static void gradient(const Tile& T, const P& p, real B, real G[3]) {
+    real dx[3], dy[3];
+    numerators(T, BulkW(), dx, dy);
+    const real n2 = T(2, 0, 0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const real s1 = (T(c, 0, 1) + T(c, 0, -1)) + (T(c, 1, 0) + T(c, -1, 0));
+      const real s2 = (T(c, 0, 2) + T(c, 0, -2)) + (T(c, 2, 0) + T(c, -2, 0));
+      G[c] = p.lap2 * s2 + (p.lap0 * T(c, 0, 0) - p.lap1 * s1);
+    }
+    const auto* kx = p.dk;
+    const auto* ky = p.dk + 3;
+    G[0] += real(2) * ((dx[1] * kx[2] - dx[2] * kx[1]) + (dy[1] * ky[2] - dy[2] * ky[1]));
+    G[1] += real(2) * ((dx[2] * kx[0] - dx[0] * kx[2]) + (dy[2] * ky[0] - dy[0] * ky[2]));
+    G[2] += real(2) * ((dx[0] * kx[1] - dx[1] * kx[0]) + (dy[0] * ky[1] - dy[1] * ky[0]));
+    G[2] -= B + p.K2 * n2;
   }
 
   // site-form energy and charge densities; wdx, wdy = the WEIGHTED numerators (halo rule R3)

@@ -43,7 +43,8 @@ class ss_params(C.Structure):
                 ("stream", C.c_void_p), ("arrest_log_capacity", C.c_int64),
                 ("integrator", C.c_int), ("flags", C.c_int),
                 ("chunks_per_segment", C.c_int), ("dmi_d", C.POINTER(C.c_double)),
-                ("mu", C.c_double), ("potential", C.c_int), ("potential_n", C.c_int)]
+                ("mu", C.c_double), ("potential", C.c_int), ("potential_n", C.c_int),
+                ("demag", C.c_double), ("demag_cycles", C.c_int)]
 
 
 _dp = C.POINTER(C.c_double)
@@ -92,8 +93,9 @@ def _check(rc, where, allow=()):
 
 
 def _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps=0, integrator=0,
-            dmi=None, mu=0.0, pot=0, potN=3):
+            dmi=None, mu=0.0, pot=0, potN=3, demag=0.0, demag_cycles=0):
     p = ss_params()
+    p.demag, p.demag_cycles = float(demag), int(demag_cycles)
     p.mu, p.potential, p.potential_n = float(mu), int(pot), int(potN)
     p.dtype, p.batch, p.dt = int(dtype), int(batch), float(dt)
     p.kappa, p.B, p.K, p.lam = float(kappa), float(B), float(K), float(lam)
@@ -122,7 +124,8 @@ class Solver:
 
     def __init__(self, theory, Nx, Ny, h, *, dtype=F64, batch=1, dt=0.0, kappa=0.0, B=0.0, K=0.0,
                  lam=0.0, B_batch=None, log_cap=0, flags=0, cps=0, integrator=RK4, dmi=None,
-                 mu=0.0, pot=POT_STANDARD, potN=3, device="cuda:0", stream=None):
+                 mu=0.0, pot=POT_STANDARD, potN=3, demag=0.0, demag_cycles=0, device="cuda:0",
+                 stream=None):
         self.theory, self.Nx, self.Ny, self.batch = int(theory), int(Nx), int(Ny), int(batch)
         self.C = 4 if theory == THEORY_ABELIAN_HIGGS else 3
         self.dtype = dtype
@@ -131,7 +134,7 @@ class Solver:
         self.device = torch.device(device)
         self._h = C.c_void_p()
         p, keep = _params(dtype, batch, dt, kappa, B, K, lam, B_batch, log_cap, flags, cps,
-                          integrator, dmi, mu, pot, potN)
+                          integrator, dmi, mu, pot, potN, demag, demag_cycles)
         nbytes = _lib.ss_workspace_bytes(self.theory, self.Nx, self.Ny, C.byref(p))
         if nbytes == 0:
             # invalid or over a limit: ss_create tells which (it checks before touching memory)
@@ -221,9 +224,10 @@ class Solver:
 
     def profile_step(self, reps=1):
         """[(kernel name, average ms)] of one flow step, kernels launched one by one."""
-        buf = (C.c_double * 16)()
+        cap = 8192                          # a demagnetisation step has a few hundred kernels
+        buf = (C.c_double * cap)()
         n = C.c_int()
-        _check(_lib.ss_profile_step(self._h, int(reps), buf, 16, C.byref(n)), "ss_profile_step")
+        _check(_lib.ss_profile_step(self._h, int(reps), buf, cap, C.byref(n)), "ss_profile_step")
         return [(_lib.ss_kernel_name(self._h, i).decode(), buf[i]) for i in range(n.value)]
 
     def _scalar(self, fn, name, strict):
@@ -276,10 +280,11 @@ class Solver:
 
 
 def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0,
-               integrator=RK4) -> Solver:
+               integrator=RK4, demag_cycles=0) -> Solver:
     """Solver configured from a workloads.Workload (sizes and parameters only)."""
     return Solver(w.theory, w.Nx, w.Ny, w.h, dtype=dtype, batch=w.batch, dt=w.dt, kappa=w.kappa,
                   B=w.B, K=w.K, lam=w.lam, B_batch=w.B_batch, log_cap=log_cap, flags=flags,
                   cps=cps, integrator=integrator, dmi=getattr(w, "dmi", None),
                   mu=getattr(w, "mu", 0.0), pot=getattr(w, "pot", 0), potN=getattr(w, "potN", 3),
+                  demag=getattr(w, "demag", 0.0), demag_cycles=demag_cycles,
                   device=device)

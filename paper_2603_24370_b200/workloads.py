@@ -43,6 +43,7 @@ class Workload:
     K: float = 0.0
     lam: float = 0.0
     mu: float = 0.0                   # baby Skyrme: V proportional to mu^2
+    demag: float = 0.0                # chiral magnet: g = mu0 Ms^2 of the demagnetisation term
     pot: int = 0                      # baby Skyrme: POT_*
     potN: int = 3                     # baby Skyrme: N of the Z_N-symmetric potential
     batch: int = 1
@@ -215,6 +216,14 @@ def bs_single(N=128, h=0.2, kappa=1.0, mu=1.0, pot=POT_STANDARD, potN=3, noise=0
 def bs_bench() -> Workload:
     """The baby-Skyrme bench workload: 2048^2, 32 hedgehogs, standard potential."""
     return bs_single(N=2048, count=32, steps=2000)
+
+
+def cm_demag_bench() -> Workload:
+    """Demagnetisation bench workload (not a BASELINE config): config 2's
+    multi-skyrmion recipe at 2048^2 with Neel DMI and g = mu0 Ms^2 = 1."""
+    w = cm_multi(N=2048, count=64, margin=12.0, min_sep=16.0)
+    w.name, w.demag, w.dmi, w.K = "cm_demag_2048", 1.0, DMI_NEEL, 0.1
+    return w
 
 
 def baseline_config(c: int, **kw) -> Workload:
