@@ -44,7 +44,7 @@ struct ResidentArgs {
 inline size_t resident_smem_doubles(int Nx, int Ny, int rows) {
   const size_t W = Nx, PS = (size_t)(rows + 4) * W, PO = (size_t)rows * W;
   return 4 * 3 * PS       // phi, S2, S3, S4 with two halo rows above and below
-         + 3 * 3 * PO     // v, a1, a2
+         + (2 * PO <= (size_t)RES_THREADS ? 4 : 3) * 3 * PO  // v, a1, a2 (+ a4 exchange, split mode)
          + 3 * (size_t)rows * (W / 32)  // per-warp partial sums of e, q, ke
          + 3 * (size_t)Ny               // all row sums of the lattice
          + 3 * 32 + 8;                  // y-tree scratch, totals
@@ -71,7 +71,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
   double* vel = S4 + 3 * PS;      // [3][RR][W]
   double* A1 = vel + 3 * PO;
   double* A2 = A1 + 3 * PO;
-  double* wsum = A2 + 3 * PO;     // [3][RR][NW]
+  double* XB = A2 + 3 * PO;       // a4 handed from role 1 to role 0 (split mode only)
+  double* wsum = XB + (2 * nsite <= RES_THREADS ? 3 * PO : 0);  // [3][RR][NW]
   double* rows_all = wsum + 3 * RR * NW;  // [3][Ny]
   double* ysh = rows_all + 3 * Ny;        // [3][32]
   double* tot = ysh + 3 * 32;     // [3] + flags
@@ -177,9 +178,19 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     }
   };
 
-  for (long long it = 0; it < a.steps; ++it) {
-    // ---- P1: stage fields phi3, phi4 of the own rows (fill_site of kernel Y)
-    for (int s = tid; s < nsite; s += RES_THREADS) {
+  // Work split.  With at most half as many sites as threads (64 x 64 on 16 CTAs: 256 sites, 512
+  // threads) every site gets TWO threads: role 0 evaluates the first stage field of a phase
+  // (phi3, then phi'), role 1 the second (phi4, then phi2'), each routine still run whole by one
+  // thread on the same inputs, so nothing changes numerically.  Otherwise one thread does both.
+  const bool split = 2 * nsite <= RES_THREADS;
+  const int mask = split ? (tid < nsite ? 1 : (tid < 2 * nsite ? 2 : 0)) : 3;
+  const int s0 = split ? (tid < nsite ? tid : tid - nsite) : tid;
+  const int sstep = split ? 2 * nsite : RES_THREADS;  // split: exactly one site per thread
+  const int send = mask ? nsite : 0;
+
+  // ---- P1: stage fields phi3 (role 0), phi4 (role 1) of the own rows (fill_site of kernel Y)
+  auto P1 = [&](bool vzz) {
+    for (int s = s0; s < send; s += sstep) {
       const int r = s / W, x = s - r * W, gy = gy0 + r;
       double A[3], Bf[3];
 #pragma unroll
@@ -189,94 +200,142 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         for (int c = 0; c < 3; ++c) {
           const double ph = A[c];
           const double a1 = A1[c * PO + s];
-          const double vh = vz ? 0.0 : vel[c * PO + s];
-          const double a2 = vz ? a1 : A2[c * PO + s];
+          const double vh = vzz ? 0.0 : vel[c * PO + s];
+          const double a2 = vzz ? a1 : A2[c * PO + s];
           A[c] = (ph + p.hdt * vh) + p.qdt2 * a1;
           const double base = ph + p.dt * vh;
           Bf[c] = base + p.hdt2 * a2;
         }
-        Th::project_field(A);
-        Th::project_field(Bf);
+        if (mask & 1) Th::project_field(A);
+        if (mask & 2) Th::project_field(Bf);
       }
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
-        put(S3, c, r, x, A[c]);
-        put(S4, c, r, x, Bf[c]);
+        if (mask & 1) put(S3, c, r, x, A[c]);
+        if (mask & 2) put(S4, c, r, x, Bf[c]);
       }
     }
-    cluster.sync();
+  };
+  // RK4 combine, projections, KE, phi2' of one site from a3 = aA, a4 = aB (kernel Y, X's fill)
+  auto combine = [&](int s, int r, int x, const double (&aA)[3], const double (&aB)[3]) -> double {
+    const int o = (r + 2) * W + x;
+    double fn[3], u[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double ph = phi[c * PS + o];
+      const double a1 = A1[c * PO + s];
+      const double vh = vz ? 0.0 : vel[c * PO + s];
+      const double a2 = vz ? a1 : A2[c * PO + s];
+      const double base = ph + p.dt * vh;
+      const double k0 = base + p.sdt2 * (a1 + a2);
+      const double k1 = vh + p.sdt * (a1 + 2.0 * a2);
+      fn[c] = k0 + p.sdt2 * aA[c];
+      u[c] = k1 + p.sdt * (2.0 * aA[c] + aB[c]);
+    }
+    Th::project_field(fn);
+    Th::project_velocity(u, fn);
+    double v2 = 0.0, B2[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      put(phi, c, r, x, fn[c]);
+      vel[c * PO + s] = u[c];
+      v2 += u[c] * u[c];
+      B2[c] = fn[c] + p.hdt * u[c];
+    }
+    Th::project_field(B2);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) put(S2, c, r, x, B2[c]);
+    return 0.5 * v2;
+  };
 
-    // ---- P2: a3, a4, RK4 combine, projections, KE; phi2' of the new state (kernel Y, X's fill)
-    for (int s = tid; s < nsite; s += RES_THREADS) {
-      const int r = s / W, x = s - r * W, gy = gy0 + r;
-      double ke = 0.0;
-      if (active_site(x, gy)) {
-        const int o = (r + 2) * W + x;
+  P1(vz);
+  cluster.sync();
+  for (long long it = 0; it < a.steps; ++it) {
+    // ---- P2: a3 (role 0), a4 (role 1), then the combine
+    if (split) {
+      const int s = s0, r = s / W, x = s - r * W, gy = gy0 + r;
+      const bool act = mask && active_site(x, gy);
+      const int o = (r + 2) * W + x;
+      double aA[3] = {0.0, 0.0, 0.0}, aB[3];
+      if (act && mask == 1) {
         auto TA = [&](int c, int dy, int dx) -> double { return S3[c * PS + o + dy * W + dx]; };
-        auto TB = [&](int c, int dy, int dx) -> double { return S4[c * PS + o + dy * W + dx]; };
-        double aA[3], aB[3], fn[3], u[3];
         Th::accel(TA, p, Bz, aA);
+      }
+      if (act && mask == 2) {
+        auto TB = [&](int c, int dy, int dx) -> double { return S4[c * PS + o + dy * W + dx]; };
         Th::accel(TB, p, Bz, aB);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          const double ph = phi[c * PS + o];
-          const double a1 = A1[c * PO + s];
-          const double vh = vz ? 0.0 : vel[c * PO + s];
-          const double a2 = vz ? a1 : A2[c * PO + s];
-          const double base = ph + p.dt * vh;
-          const double k0 = base + p.sdt2 * (a1 + a2);
-          const double k1 = vh + p.sdt * (a1 + 2.0 * a2);
-          fn[c] = k0 + p.sdt2 * aA[c];
-          u[c] = k1 + p.sdt * (2.0 * aA[c] + aB[c]);
-        }
-        Th::project_field(fn);
-        Th::project_velocity(u, fn);
-        double v2 = 0.0, B2[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          put(phi, c, r, x, fn[c]);
-          vel[c * PO + s] = u[c];
-          v2 += u[c] * u[c];
-          B2[c] = fn[c] + p.hdt * u[c];
-        }
-        Th::project_field(B2);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) put(S2, c, r, x, B2[c]);
-        ke = 0.5 * v2;
-      } else {  // frozen halo: phi2' = phi there (the neighbours' copies of phi never change)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) put(S2, c, r, x, phi[c * PS + (r + 2) * W + x]);
+        for (int c = 0; c < 3; ++c) XB[c * PO + s] = aB[c];
       }
-      warp_sums(s, ke, 0.0, 1, 2);
+      __syncthreads();
+      if (mask == 1) {
+        double ke = 0.0;
+        if (act) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) aB[c] = XB[c * PO + s];
+          ke = combine(s, r, x, aA, aB);
+        } else {  // frozen halo: phi2' = phi there (the neighbours' copies of phi never change)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) put(S2, c, r, x, phi[c * PS + o]);
+        }
+        warp_sums(s, ke, 0.0, 1, 2);
+      }
+    } else {
+      for (int s = s0; s < send; s += sstep) {
+        const int r = s / W, x = s - r * W, gy = gy0 + r;
+        double ke = 0.0;
+        if (active_site(x, gy)) {
+          const int o = (r + 2) * W + x;
+          auto TA = [&](int c, int dy, int dx) -> double { return S3[c * PS + o + dy * W + dx]; };
+          auto TB = [&](int c, int dy, int dx) -> double { return S4[c * PS + o + dy * W + dx]; };
+          double aA[3], aB[3];
+          Th::accel(TA, p, Bz, aA);
+          Th::accel(TB, p, Bz, aB);
+          ke = combine(s, r, x, aA, aB);
+        } else {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) put(S2, c, r, x, phi[c * PS + (r + 2) * W + x]);
+        }
+        warp_sums(s, ke, 0.0, 1, 2);
+      }
     }
     cluster.sync();
 
-    // ---- P3: a1, e, q on phi'; a2 on phi2' (kernel X)
-    for (int s = tid; s < nsite; s += RES_THREADS) {
+    // ---- P3: a1, e, q on phi' (role 0); a2 on phi2' (role 1)  (kernel X)
+    for (int s = s0; s < send; s += sstep) {
       const int r = s / W, x = s - r * W, gy = gy0 + r;
-      double e = 0.0, q = 0.0;
-      if (active_site(x, gy)) {
-        const int o = (r + 2) * W + x;
-        auto TA = [&](int c, int dy, int dx) -> double { return phi[c * PS + o + dy * W + dx]; };
-        auto TB = [&](int c, int dy, int dx) -> double { return S2[c * PS + o + dy * W + dx]; };
-        double aA[3], aB[3];
-        if (x < 2 * HALO || x >= Nx - 2 * HALO || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
-          Th::accel(TA, p, Bz, aA);
-          Th::densities(TA, p, Bz, EdgeW(x, gy, Nx, Ny), e, q);
-        } else {
-          Th::accel_densities_bulk(TA, p, Bz, aA, e, q);
+      const bool act = active_site(x, gy);
+      const int o = (r + 2) * W + x;
+      if (mask & 1) {
+        double e = 0.0, q = 0.0;
+        if (act) {
+          auto TA = [&](int c, int dy, int dx) -> double { return phi[c * PS + o + dy * W + dx]; };
+          double aA[3];
+          if (x < 2 * HALO || x >= Nx - 2 * HALO || gy < 2 * HALO || gy >= Ny - 2 * HALO) {
+            Th::accel(TA, p, Bz, aA);
+            Th::densities(TA, p, Bz, EdgeW(x, gy, Nx, Ny), e, q);
+          } else {
+            Th::accel_densities_bulk(TA, p, Bz, aA, e, q);
+          }
+#pragma unroll
+          for (int c = 0; c < 3; ++c) A1[c * PO + s] = aA[c];
         }
+        warp_sums(s, e, q, 2, 0);
+      }
+      if ((mask & 2) && act) {
+        auto TB = [&](int c, int dy, int dx) -> double { return S2[c * PS + o + dy * W + dx]; };
+        double aB[3];
         Th::accel(TB, p, Bz, aB);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          A1[c * PO + s] = aA[c];
-          A2[c * PO + s] = aB[c];
-        }
+        for (int c = 0; c < 3; ++c) A2[c * PO + s] = aB[c];
       }
-      warp_sums(s, e, q, 2, 0);
     }
     __syncthreads();
     row_sums();
+    // the next step's stage fields, assuming this step is not arrested (the common case): their
+    // pushes travel under the same cluster barrier as the row sums
+    const bool more = it + 1 < a.steps;
+    if (more) P1(false);
     cluster.sync();
 
     // ---- P4: canonical y-tree, E, Q, KE, arrest (finalize_kernel), in every CTA
@@ -302,6 +361,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
       vz = arrest;
     }
     __syncthreads();  // tot is rewritten by the next step
+    if (vz && more) {  // arrested (every CTA takes the same decision): redo the stage fields
+      P1(true);
+      cluster.sync();
+    }
   }
 
   // ---- store the state
