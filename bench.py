@@ -413,7 +413,14 @@ def run_ours(args):
             t = ncu_traffic(args.workload, args.integrator, n)
             kern[n]["traffic"] = t["bytes"] if t else None
     tr = ncu_traffic(args.workload, args.integrator, dom)
+    note = None
+    if s.schedule() == "resident-cluster":
+        note = ("ss_step runs the resident-cluster schedule (one launch for all steps, state in "
+                "shared memory: nothing streams from HBM, no HBM roofline applies); the kernels "
+                "listed here are the general two-kernel schedule of the same solver, launched one "
+                "by one by ss_profile_step, for comparison")
     roofline = {
+        "note": note,
         "bound": "hbm", "limiter": kern[dom]["limiter"],
         "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak,
         "unit": "GB/s", "frac": kern[dom]["gbs"] / peak,
