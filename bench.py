@@ -282,7 +282,7 @@ def ncu_traffic(workload_key, integrator, kernel):
     return None
 
 
-DEMAG_DEFAULT_CYCLES = 12                       # include/ss.h: demag_cycles = 0
+DEMAG_DEFAULT_CYCLES = 8                        # include/ss.h: demag_cycles = 0
 
 
 def mg_alg_bytes(w, cycles):

@@ -107,8 +107,8 @@ typedef struct {
                            /* (g/2)|grad psi|^2, lap psi = d1 n1 + d2 n2, psi = 0 on the halo         */
                            /* (PAPER.md:196 eq. 5, :199-203 eq. 6; DESIGN R19); 0 = off.  Needs       */
                            /* SS_VERLET and SS_F64; psi is solved by multigrid V-cycles on the device */
-  int demag_cycles;        /* V-cycles per step, warm-started (0 -> 12; 4x as many in ss_set_fields); */
-                           /* contraction per cycle 0.27 (even sizes on every level) ... 0.65        */
+  int demag_cycles;        /* V-cycles per step, warm-started (0 -> 8; 4x as many in ss_set_fields);  */
+                           /* measured contraction per cycle 0.27                                     */
 } ss_params;
 
 /* Limits of this build: 5 <= Nx <= 65536, 5 <= Ny <= 32768 (the device-side reduction tree of

@@ -406,9 +406,19 @@ void add_vcycle(const ss_solver* s, size_t l, std::vector<KernelNode>& out) {
   MgArgs m;
   memset(&m, 0, sizeof(m));
   m.nx = f.nx; m.ny = f.ny; m.c = f.c; m.rhs = rhs;
-  {  // wall factor alpha_l = (1 - d_l)/d_l, d_l = 1/2 + 1/2^(l+1); 0 on the lattice itself
-    const double d = 0.5 + 0.5 / double(1 << l);
-    m.alpha = l == 0 ? 0.0 : (1.0 - d) / d;
+  if (l > 0) {  // wall images: psi(-k) = (d - k)/d psi(0), d = distance of the wall-adjacent unknown
+    m.walls = 1;   // from the physical wall in spacings of this level (ss_demag.cuh mg_store)
+    const double sp = double(1 << l);
+    const double dl = 0.5 + 0.5 / sp;  // unknown I of level l sits at 2^l I + (2^l - 1)/2 fine cells
+    const double n0[2] = {double(s->L.mg[0].nx), double(s->L.mg[0].ny)};
+    const int nl[2] = {f.nx, f.ny};
+    for (int dim = 0; dim < 2; ++dim) {
+      const double dr = (n0[dim] - (sp * (nl[dim] - 1) + (sp - 1.0) / 2.0)) / sp;
+      for (int k = 1; k <= 2; ++k) {
+        m.bw[4 * dim + k - 1] = (dl - k) / dl;
+        m.bw[4 * dim + 2 + k - 1] = (dr - k) / dr;
+      }
+    }
   }
   if (l + 1 == s->L.mg.size()) {
     m.out = psi;
@@ -681,7 +691,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   s->theory = theory; s->dtype = p->dtype; s->C = theory == SS_THEORY_ABELIAN_HIGGS ? 4 : 3;
   s->mu = p->mu; s->pot = p->potential; s->potN = p->potential_n;
   s->demag = theory == SS_THEORY_CHIRAL_MAGNET ? p->demag : 0.0;
-  s->demag_cycles = p->demag_cycles > 0 ? p->demag_cycles : 12;
+  s->demag_cycles = p->demag_cycles > 0 ? p->demag_cycles : 8;
   s->Nx = Nx; s->Ny = Ny; s->batch = p->batch; s->h = h;
   s->device = pa.device;
   s->dt = p->dt > 0.0 ? p->dt : 0.5 * h;

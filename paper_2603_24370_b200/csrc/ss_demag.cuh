@@ -9,9 +9,10 @@
 //                        damped-Jacobi smoothing of the 4th-order operator (omega = 10/13, the
 //                        optimum for its symbol: smoothing factor 0.64), cell-centred
 //                        coarsening by 2 (4-point averaging down, bilinear up; an odd size drops
-//                        its last cell: n_c = floor(n/2), so the coarse wall never lies outside
-//                        the fine one), the same eq. (2) operator with h_l = 2^l h on every
-//                        level, coarsest level (<= 8 x 8) relaxed to convergence by one CTA
+//                        its last cell: n_c = floor(n/2)), the same eq. (2) operator with
+//                        h_l = 2^l h on every level, each coarse level closed by wall images at
+//                        its exact distance from the physical wall, coarsest level (<= 8 x 8)
+//                        relaxed to convergence by one CTA
 //   demag_kick_kernel    a' = -Pi(G(phi') + g (D_x psi, D_y psi, 0)), e_i + g x bond density of
 //                        psi, q_i, v' = Pi(w + dt/2 a'), KE, row-segment partial sums
 //
@@ -39,30 +40,37 @@ struct MgArgs {
   int nx, ny;         // fine (or only) level
   int cnx, cny;       // coarse level
   double c;           // 1 / (12 h_l^2) of the level the operator is applied on
-  double alpha;       // wall factor of the level the output lives on (see mg_store); 0 on level 0
-  double calpha;      // restrict: wall factor of the coarse level
+  int walls;          // 0 on level 0 (plain zero halo); 1: the level's halo holds wall images
+  double bw[8];       // image factors of the output level: (beta1, beta2) for the left, right,
+                      // bottom and top wall (see mg_store)
 };
 
 // Wall treatment.  Level 0 is the lattice: psi = 0 on its two halo layers (the wall sits on the
-// first halo node, one spacing from the first unknown).  The first unknown of a cell-centred
-// coarse level l >= 1 lies d_l = 1/2 + 1/2^(l+1) of ITS spacing from that wall (0.75, 0.63, ... ->
-// 0.5).  Its two halo layers hold the images psi(-1) = -alpha psi(0), psi(-2) = -alpha psi(1),
-// alpha_l = (1 - d_l)/d_l: the straight line through the wall for the first image (alpha = 0 on
-// level 0: plain zeros; alpha -> 1: antisymmetric reflection about the cell face).  Whoever
-// writes cell (i, j) of a level also writes its images (corners: both factors).
+// first halo node, one spacing from the first unknown).  On a cell-centred coarse level l >= 1 the
+// first / last unknown lies d spacings OF THAT LEVEL from the same physical wall -- d = 1/2 +
+// 1/2^(l+1) on the left and bottom, and on the right and top whatever the dropped cells of the
+// odd sizes above leave (1.0 ... 1.25 right after a drop).  Its two halo layers hold the values of
+// the straight line through the wall and the wall-adjacent unknown: psi(-k) = beta_k psi(0),
+// beta_k = (d - k)/d.  Whoever writes a wall-adjacent cell of such a level also writes its
+// images (corners: the product), so every kernel reads plain neighbours.
 __device__ __forceinline__ void mg_store(double* q, int i, int j, int nx, int ny, int pitch,
-                                         double v, double alpha) {
+                                         double v, int walls, const double* bw) {
   q[0] = v;
-  if (alpha == 0.0) return;
-  const int mx = i < 2 ? -(2 * i + 1) : (i >= nx - 2 ? 2 * (nx - 1 - i) + 1 : 0);
-  const int my = j < 2 ? -(2 * j + 1) : (j >= ny - 2 ? 2 * (ny - 1 - j) + 1 : 0);
-  const double w = -alpha * v;
-  if (mx) q[mx] = w;
-  if (my) q[my * pitch] = w;
-  if (mx && my) q[my * pitch + mx] = -alpha * w;
-  // a level only 2 or 3 cells wide: cell i can be within two cells of BOTH walls
-  if (i < 2 && i >= nx - 2) q[2 * (nx - 1 - i) + 1] = w;
-  if (j < 2 && j >= ny - 2) q[(2 * (ny - 1 - j) + 1) * pitch] = w;
+  if (!walls) return;
+  const bool L = i == 0, R = i == nx - 1, B = j == 0, T = j == ny - 1;
+  if (!(L || R || B || T)) return;
+#pragma unroll
+  for (int k = 1; k <= 2; ++k) {
+    if (L) q[-k] = bw[k - 1] * v;
+    if (R) q[k] = bw[2 + k - 1] * v;
+    if (B) q[-k * pitch] = bw[4 + k - 1] * v;
+    if (T) q[k * pitch] = bw[6 + k - 1] * v;
+  }
+  // corners, read only by the bilinear prolongation from this level (nearest image only)
+  if (L && B) q[-pitch - 1] = bw[0] * bw[4] * v;
+  if (R && B) q[-pitch + 1] = bw[2] * bw[4] * v;
+  if (L && T) q[pitch - 1] = bw[0] * bw[6] * v;
+  if (R && T) q[pitch + 1] = bw[2] * bw[6] * v;
 }
 
 __device__ __forceinline__ double mg_lap(const double* q, int pitch, double c) {
@@ -84,7 +92,7 @@ __global__ void __launch_bounds__(MGX* MGY) mg_smooth_kernel(const __grid_consta
   const int pitch = nx + 4;
   const long long o = ((long long)blockIdx.z * (ny + 4) + j + 2) * pitch + i + 2;
   const double r = rhs[o] - mg_lap(in + o, pitch, c);
-  mg_store(out + o, i, j, nx, ny, pitch, in[o] - (MG_OMEGA / (60.0 * c)) * r, m.alpha);
+  mg_store(out + o, i, j, nx, ny, pitch, in[o] - (MG_OMEGA / (60.0 * c)) * r, m.walls, m.bw);
 }
 
 // coarse rhs = average of the residuals of the four fine children; coarse psi = 0
@@ -109,7 +117,7 @@ __global__ void __launch_bounds__(MGX* MGY) mg_restrict_kernel(const __grid_cons
     }
   const long long co = ((long long)blockIdx.z * (cny + 4) + J + 2) * (cnx + 4) + I + 2;
   crhs[co] = 0.25 * s;
-  mg_store(cpsi + co, I, J, cnx, cny, cnx + 4, 0.0, 1.0);  // zero the stale images too
+  mg_store(cpsi + co, I, J, cnx, cny, cnx + 4, 0.0, 1, m.bw);  // zero the stale images too
 }
 
 // psi_fine += bilinear (cell-centred) interpolation of the coarse correction (the last cell of an
@@ -147,14 +155,14 @@ __global__ void __launch_bounds__(1024) mg_coarse_kernel(const __grid_constant__
     for (int k = threadIdx.x; k < nx * ny; k += blockDim.x) {
       const int o = (k / nx + 2) * pitch + k % nx + 2;
       mg_store(b2 + o, k % nx, k / nx, nx, ny, pitch,
-               a[o] - (MG_OMEGA / (60.0 * c)) * (r[o] - mg_lap(a + o, pitch, c)), m.alpha);
+               a[o] - (MG_OMEGA / (60.0 * c)) * (r[o] - mg_lap(a + o, pitch, c)), m.walls, m.bw);
     }
     __syncthreads();
     double* t = a; a = b2; b2 = t;
   }
   for (int k = threadIdx.x; k < nx * ny; k += blockDim.x) {
     const int o = (k / nx + 2) * pitch + k % nx + 2;
-    mg_store(psi + base + o, k % nx, k / nx, nx, ny, pitch, a[o], m.alpha);
+    mg_store(psi + base + o, k % nx, k / nx, nx, ny, pitch, a[o], m.walls, m.bw);
   }
 }
 
