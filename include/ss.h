@@ -8,7 +8,10 @@
  *     stencils of PAPER.md:100-109 (eq. 1, eq. 2);
  *   - the discretised energy E_h, its exact gradient and the topological charge of
  *       SS_THEORY_CHIRAL_MAGNET  n in S^2:  1/2|grad n|^2 + kappa n.(curl n) + B(1-n3) + K(1-n3^2)
- *                                (PAPER.md:196 eq. 5, :327; DESIGN R1-R3),
+ *                                (PAPER.md:196 eq. 5, :327; DESIGN R1-R3); optionally the DMI
+ *                                term as kappa sum_mu d_mu.(n x d_mu n) with a table (dmi_d,
+ *                                DESIGN R16) and the magnetostatic energy (g/2)|grad psi|^2,
+ *                                lap psi = div n (demag; eq. 5-6; DESIGN R19),
  *       SS_THEORY_ABELIAN_HIGGS  phi in C, A in R^2: 1/2|D phi|^2 + 1/2 (curl A)^2
  *                                + (lambda/8)(1-|phi|^2)^2   (DESIGN R1-R3, R9),
  *       SS_THEORY_BABY_SKYRME    m in S^2: 1/2|grad m|^2 + (kappa^2/2)|d1 m x d2 m|^2 + V(m)
@@ -25,7 +28,7 @@
  *             Interior = 2 <= i < Nx-2, 2 <= j < Ny-2.  Halo sites are frozen: supplied by
  *             ss_set_fields and never written by a step.
  *   Layout    field arrays are dense [batch][C][Ny][Nx] of `real` (double for SS_F64, float
- *             for SS_F32), x fastest.  C = 3 (n1,n2,n3) for the chiral magnet, C = 4
+ *             for SS_F32), x fastest.  C = 3 (n1,n2,n3) for the chiral magnet and baby Skyrme, C = 4
  *             (Re phi, Im phi, A1, A2) for Abelian Higgs.  Velocities have the same shape;
  *             their halo entries are ignored on input and written as 0 on output.
  *   Memory    every pointer named *_dev is DEVICE memory owned by the caller; every pointer

@@ -112,3 +112,15 @@ def test_demag_zero_coupling_equals_plain_verlet_and_unsupported_combinations():
         s.step(30)
     assert np.abs((a.get_fields()[0] - b.get_fields()[0]).cpu().numpy()).max() < 1e-12
     assert a.arrests(0) == b.arrests(0)
+
+
+def test_paper_usage_example_shape_antiskyrmion_with_demag():
+    """The paper's usage example (Fig. 1-2): a 320 x 320 lattice, D2d
+    ("Heusler") DMI with the antiskyrmion ansatz, demagnetisation on, stepped five steps per
+    frame.  (Its physical units and newtonflow=False are not reproduced: DESIGN R16, R19.)  Four
+    frames of ss_step(5) against the oracle; the texture is an antiskyrmion, Q = +1."""
+    w = W.cm_single(N=320, K=0.1, mirror=True)
+    w.dmi, w.demag = W.DMI_D2D, 0.5
+    s, fl, _ = _run(w, (5, 10, 15, 20), cycles=24, ftol=1e-10, etol=1e-9)
+    assert abs(s.charge()[0] - 1.0) < 5e-3
+    assert fl.energy < oracle.energy_charge(_model(w), w.fields[0])[0]
