@@ -80,27 +80,68 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
     return gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO;
   };
 
-  // ---- phase 1: stage field on the tile + 4
-  for (int idx = tid; idx < BMY * BMX; idx += BBX * BBY) {
-    const int ly = idx / BMX, lx = idx - ly * BMX;
-    const int gx = x0 - BH + lx, gy = y0 - BH + ly;
-    real m[3] = {real(0), real(0), real(0)};
-    if (gx >= 0 && gx < Nx && gy >= 0 && gy < Ny) {
-      const long long o = (long long)gy * Nx + gx;
+  // ---- phase 1: stage field on the tile + 4.  A thread owns NS1 sites; all loads of one input
+  // array are issued before any is used (27 independent loads in flight per thread and array:
+  // the tile is read at L2 latency once, not once per site)
+  constexpr int NS1 = (BMY * BMX + BBX * BBY - 1) / (BBX * BBY);
+  {
+    long long off[NS1];
+    bool in[NS1], inter[NS1];
+    real m[NS1][3];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) m[c] = phi[c * p.plane + o];
-      if (STAGE > 1 && interior(gx, gy)) {  // halo sites of every stage field are the frozen halo
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          const real vh = vz ? real(0) : vel[c * p.plane + o];
-          m[c] = m[c] + p.alpha * vh;
-          if (STAGE > 2) m[c] = m[c] + p.beta * aprev[c * p.plane + o];
-        }
-        Th::project_field(m);
-      }
+    for (int k = 0; k < NS1; ++k) {
+      const int idx = tid + k * BBX * BBY;
+      const int ly = idx / BMX, lx = idx - ly * BMX;
+      const int gx = x0 - BH + lx, gy = y0 - BH + ly;
+      in[k] = idx < BMY * BMX && gx >= 0 && gx < Nx && gy >= 0 && gy < Ny;
+      inter[k] = in[k] && interior(gx, gy);
+      off[k] = in[k] ? (long long)gy * Nx + gx : 0;
     }
 #pragma unroll
-    for (int c = 0; c < 3; ++c) sm.m[c][ly][lx] = m[c];
+    for (int k = 0; k < NS1; ++k)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) m[k][c] = in[k] ? phi[c * p.plane + off[k]] : real(0);
+    if (STAGE > 1) {  // halo sites of every stage field are the frozen halo
+      if (!vz) {
+        real v[NS1][3];
+#pragma unroll
+        for (int k = 0; k < NS1; ++k)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) v[k][c] = inter[k] ? vel[c * p.plane + off[k]] : real(0);
+#pragma unroll
+        for (int k = 0; k < NS1; ++k)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) m[k][c] = m[k][c] + p.alpha * v[k][c];
+      } else {
+#pragma unroll
+        for (int k = 0; k < NS1; ++k)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) m[k][c] = m[k][c] + p.alpha * real(0);
+      }
+      if (STAGE > 2) {
+        real ap[NS1][3];
+#pragma unroll
+        for (int k = 0; k < NS1; ++k)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) ap[k][c] = inter[k] ? aprev[c * p.plane + off[k]] : real(0);
+#pragma unroll
+        for (int k = 0; k < NS1; ++k)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) m[k][c] = m[k][c] + p.beta * ap[k][c];
+      }
+#pragma unroll
+      for (int k = 0; k < NS1; ++k)
+        if (inter[k]) Th::project_field(m[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < NS1; ++k) {
+      const int idx = tid + k * BBX * BBY;
+      if (idx < BMY * BMX) {
+        const int ly = idx / BMX, lx = idx - ly * BMX;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sm.m[c][ly][lx] = m[k][c];
+      }
+    }
   }
   __syncthreads();
 
