@@ -252,6 +252,12 @@ KERNEL_UNITS = {
     # planes and are reported by their time only
     "demag_drift": 5,
     "demag_kick_energy_charge_ke": 13.0 / 3.0,
+    # RK4 with demagnetisation: per stage S = R(phi + ..) (reads phi, v, a_prev, writes S), the
+    # stage acceleration (reads S, psi, writes a), then the combine (reads phi, v, a1..a4, writes
+    # phi', v'); summed over the three launches per step each
+    "demag_stage_field": 3 + 3 + 4,
+    "demag_stage_accel": 3 * (2 + 1.0 / 3.0),
+    "demag_rk4_combine_project_ke": 8,
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
@@ -295,7 +301,7 @@ def ncu_traffic(workload_key, integrator, kernel):
 DEMAG_DEFAULT_CYCLES = 8                        # include/ss.h: demag_cycles = 0
 
 
-def mg_alg_bytes(w, cycles):
+def mg_alg_bytes(w, cycles, solves=1):
     """Algorithmic bytes per step of the multigrid kernels (csrc/ss_demag.cuh header): per
     V-cycle and level 4 sweeps x (read psi, rhs; write psi), one residual + restriction (read psi,
     rhs; write 1/4 rhs, 1/4 psi), one prolongation (read psi, 1/4 coarse; write psi), fp64."""
@@ -306,8 +312,9 @@ def mg_alg_bytes(w, cycles):
             break
         nx, ny = nx // 2, ny // 2
     fine = sum(sizes[:-1]) * w.batch
-    return {"mg_smooth": cycles * 4 * 24 * fine, "mg_residual_restrict": cycles * 20 * fine,
-            "mg_prolong_add": cycles * 18 * fine, "demag_rho": 24 * sizes[0] * w.batch}
+    n = cycles * solves
+    return {"mg_smooth": n * 4 * 24 * fine, "mg_residual_restrict": n * 20 * fine,
+            "mg_prolong_add": n * 18 * fine, "demag_rho": solves * 24 * sizes[0] * w.batch}
 
 
 def max_over_ranks(values, dist=None, device="cpu"):
@@ -404,7 +411,8 @@ def run_ours(args):
         t = agg.setdefault(name, [0.0, 0])
         t[0] += kms
         t[1] += 1
-    mg = mg_alg_bytes(w, DEMAG_DEFAULT_CYCLES) if getattr(w, "demag", 0.0) else {}
+    mg = mg_alg_bytes(w, DEMAG_DEFAULT_CYCLES, 1 if args.integrator == "verlet" else 4) \
+        if getattr(w, "demag", 0.0) else {}
     for name, (kms, cnt) in agg.items():
         u = KERNEL_UNITS.get(name)
         kern[name] = {"ms": kms, "launches_per_step": cnt}

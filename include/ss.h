@@ -109,8 +109,9 @@ typedef struct {
   double demag;            /* chiral magnet: g = mu0 Ms^2 >= 0 of the magnetostatic energy           */
                            /* (g/2)|grad psi|^2, lap psi = d1 n1 + d2 n2, psi = 0 on the halo         */
                            /* (PAPER.md:196 eq. 5, :199-203 eq. 6; DESIGN R19); 0 = off.  Needs       */
-                           /* SS_VERLET and SS_F64; psi is solved by multigrid V-cycles on the device */
-  int demag_cycles;        /* V-cycles per step, warm-started (0 -> 8; 4x as many in ss_set_fields);  */
+                           /* SS_F64; psi is solved by multigrid V-cycles on the device: one solve    */
+                           /* per step with SS_VERLET, one per RK4 stage field (four) with SS_RK4     */
+  int demag_cycles;        /* V-cycles per solve, warm-started (0 -> 8; 4x as many in ss_set_fields);  */
                            /* measured contraction per cycle 0.27                                     */
 } ss_params;
 

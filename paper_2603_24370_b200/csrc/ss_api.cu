@@ -50,7 +50,7 @@ struct Layout {
   size_t rows_bytes;   // [batch][3][Ny]
   size_t state_bytes, log_bytes, bb_bytes, render_bytes;
   int nacc;            // acceleration arrays: a1, a2 (+ a3 for the baby-Skyrme stage kernels)
-  size_t off_phi[2], off_vel[2], off_a[3], off_part[3], off_rows, off_state, off_log, off_bb;
+  size_t off_phi[2], off_vel[2], off_a[4], off_part[3], off_rows, off_state, off_log, off_bb;
   size_t off_render;   // ss_render scratch: block extrema of one lattice, extrema, flag
   std::vector<MgHostLevel> mg;  // demagnetisation: multigrid hierarchy (level 0 = the lattice)
   size_t off_mg, mg_bytes;
@@ -87,6 +87,8 @@ Layout make_layout(int theory, int Nx, int Ny, const ss_params* p) {
   const int C = theory == SS_THEORY_ABELIAN_HIGGS ? 4 : 3;
   const size_t R = p->dtype == SS_F64 ? 8 : 4;
   L.nacc = theory == SS_THEORY_BABY_SKYRME ? 3 : 2;  // the per-stage schedule stores a3 as well
+  if (theory == SS_THEORY_CHIRAL_MAGNET && p->demag != 0.0 && p->integrator == SS_RK4)
+    L.nacc = 4;                                       // RK4 with one Poisson solve per stage
   const size_t cap = p->arrest_log_capacity > 0 ? (size_t)p->arrest_log_capacity : 4096;
   L.nseg = (Nx + SEG - 1) / SEG;
   L.field_bytes = align_up((size_t)p->batch * C * Ny * Nx * R);
@@ -470,7 +472,39 @@ void make_demag_step(const ss_solver* s, int cur, std::vector<KernelNode>& st,
     n.args.assign((const unsigned char*)&x, (const unsigned char*)&x + sizeof(x));
     return n;
   };
-  {  // one step
+  if (s->integrator == SS_RK4) {  // one Poisson solve per stage field (ss_demag.cuh header)
+    const FlowArgs<double>& k = a.p;
+    double* S = (double*)s->phi(cur ^ 1);  // stage fields live where phi' goes at the end
+    for (int stage = 2; stage <= 4; ++stage) {
+      DemagStepArgs x = a;
+      x.d.phi = (const double*)s->phi(cur); x.d.vel = (const double*)s->vel(cur);
+      x.d.acc = stage == 3 ? (const double*)s->acc(0) : (const double*)s->acc(1);
+      x.d.use_acc = stage > 2;
+      x.d.alpha = stage == 4 ? k.dt : k.hdt;
+      x.d.beta = stage == 3 ? k.qdt2 : k.hdt2;
+      x.d.phi_out = S;
+      st.push_back(node((void*)demag_stage_kernel, x, pgrid, dim3(256, 1, 1), "demag_stage_field"));
+      x.d.phi = S;
+      st.push_back(node((void*)demag_rho_kernel, x, pgrid, dim3(256, 1, 1), "demag_rho"));
+      for (int c = 0; c < s->demag_cycles; ++c) add_vcycle(s, 0, st);
+      x.d.acc_out = (double*)s->acc(stage - 1);
+      x.d.advance = 2;
+      st.push_back(node(kick, x, kgrid, dim3(DBX, DBY, 1), "demag_stage_accel"));
+    }
+    DemagStepArgs x = a;
+    x.d.phi = (const double*)s->phi(cur); x.d.vel = (const double*)s->vel(cur);
+    x.d.a1 = (const double*)s->acc(0); x.d.a2 = (const double*)s->acc(1);
+    x.d.a3 = (const double*)s->acc(2); x.d.a4 = (const double*)s->acc(3);
+    x.d.phi_out = (double*)s->phi(cur ^ 1); x.d.vel_out = (double*)s->vel(cur ^ 1);
+    st.push_back(node((void*)demag_combine_kernel, x, kgrid, dim3(DBX, DBY, 1),
+                      "demag_rk4_combine_project_ke"));
+    x.d.phi = (const double*)s->phi(cur ^ 1);
+    st.push_back(node((void*)demag_rho_kernel, x, pgrid, dim3(256, 1, 1), "demag_rho"));
+    for (int c = 0; c < s->demag_cycles; ++c) add_vcycle(s, 0, st);
+    x.d.acc_out = (double*)s->acc(0);
+    x.d.advance = 0;
+    st.push_back(node(kick, x, kgrid, dim3(DBX, DBY, 1), "demag_kick_energy_charge_ke"));
+  } else {  // one Verlet step
     DemagStepArgs x = a;
     x.d.phi = (const double*)s->phi(cur); x.d.vel = (const double*)s->vel(cur);
     x.d.acc = (const double*)s->acc(cur);
@@ -489,7 +523,7 @@ void make_demag_step(const ss_solver* s, int cur, std::vector<KernelNode>& st,
     x.d.phi = (const double*)s->phi(cur);
     ev.push_back(node((void*)demag_rho_kernel, x, pgrid, dim3(256, 1, 1), "demag_rho"));
     for (int c = 0; c < 4 * s->demag_cycles; ++c) add_vcycle(s, 0, ev);
-    x.d.acc_out = (double*)s->acc(cur);
+    x.d.acc_out = (double*)s->acc(s->integrator == SS_RK4 ? 0 : cur);
     x.d.advance = 0;
     ev.push_back(node(kick, x, kgrid, dim3(DBX, DBY, 1), "demag_kick_energy_charge_ke"));
   }
@@ -576,7 +610,7 @@ int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* e
 // whose state fits in the shared memory of one cluster and whose clusters fit on the device at once
 void choose_resident(ss_solver* s) {
   s->res_cl = 0;
-  if (s->ktheory != kCM || s->dtype != SS_F64 || s->integrator != SS_RK4) return;
+  if (s->ktheory != kCM || s->dtype != SS_F64 || s->integrator != SS_RK4 || s->demag != 0.0) return;
   if (s->flags & SS_FLAG_NO_RESIDENT) return;
   if (s->Nx % 32 != 0 || s->Nx > 1024 || s->Ny > RES_MAX_NY) return;
   const int order[5] = {16, 8, 4, 2, 1};  // most SMs first: the fp64 pipes bound the step
@@ -667,9 +701,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (theory == SS_THEORY_BABY_SKYRME && (p->integrator != SS_RK4 || p->dmi_d))
     return SS_ERR_UNSUPPORTED;  // the baby-Skyrme kernels exist for the RK4 step only
   if (!std::isfinite(p->demag) || p->demag < 0.0 || p->demag_cycles < 0) return SS_ERR_ARG;
-  if (p->demag != 0.0 && theory == SS_THEORY_CHIRAL_MAGNET &&
-      (p->integrator != SS_VERLET || p->dtype != SS_F64))
-    return SS_ERR_UNSUPPORTED;  // demagnetisation: fp64, one-gradient-per-step integrator only
+  if (p->demag != 0.0 && theory == SS_THEORY_CHIRAL_MAGNET && p->dtype != SS_F64)
+    return SS_ERR_UNSUPPORTED;  // demagnetisation: fp64 only
   if (p->dmi_d)
     for (int i = 0; i < 6; ++i)
       if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;

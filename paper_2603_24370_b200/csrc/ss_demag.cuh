@@ -15,6 +15,10 @@
 //                        relaxed to convergence by one CTA
 //   demag_kick_kernel    a' = -Pi(G(phi') + g (D_x psi, D_y psi, 0)), e_i + g x bond density of
 //                        psi, q_i, v' = Pi(w + dt/2 a'), KE, row-segment partial sums
+// and the RK4 step with one solve per stage field: for stages 2, 3, 4
+// demag_stage_kernel (S = R(phi + alpha vh + beta a_prev)) -> demag_rho -> V-cycles -> demag_kick
+// (acceleration only), then demag_combine_kernel (phi', v', KE) and rho -> V-cycles -> kick (a1,
+// e, q) on phi'.  psi is warm-started from the previous solve throughout.
 //
 // Roofline (stated before the kernels were written): HBM, but not 10 C R.  Per
 // interior site and step in fp64: drift 5 C R = 120 B, rho 3 R = 24 B, kick 13 R = 104 B, and
@@ -181,8 +185,15 @@ struct DemagArgs {
   double* part_ke;
   const LatticeState* state;
   const double* Bb;
-  int advance;         // kick: 1 = second half kick + KE; 0 = evaluation only (ss_set_fields)
+  int advance;         // kick: 1 = second half kick + KE; 0 = evaluation (a, e, q); 2 = a only
   double g;            // mu0 Ms^2
+  // RK4 with demagnetisation (one Poisson solve per stage field)
+  const double* a1;    // combine: the four stage accelerations
+  const double* a2;
+  const double* a3;
+  const double* a4;
+  double alpha, beta;  // stage: S = R(phi + alpha vh + beta acc)
+  int use_acc;         // stage: 0 for stage 2 (no acceleration term)
 };
 struct DemagStepArgs {
   FlowArgs<double> p;  // per-site constants (tensor maps unused)
@@ -214,6 +225,32 @@ __global__ void __launch_bounds__(256) demag_drift_kernel(const __grid_constant_
     d.phi_out[lat + c * p.plane + i] = m[c];
     d.vel_out[lat + c * p.plane + i] = w[c];
   }
+}
+
+// RK4 stage field S = R(phi + alpha vh [+ beta a_prev]) on the interior (PAPER.md:123, :129+154;
+// the same expressions as the oracle's stage_field), written where phi' will go later
+__global__ void __launch_bounds__(256) demag_stage_kernel(const __grid_constant__ DemagStepArgs A) {
+  const FlowArgs<double>& p = A.p;
+  const DemagArgs& d = A.d;
+  const int Nx = p.Nx, Ny = p.Ny;
+  const int b = blockIdx.z;
+  const bool vz = d.state[b].v_is_zero != 0;
+  const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (i >= p.plane) return;
+  const int x = int(i % Nx), y = int(i / Nx);
+  if (x < HALO || x >= Nx - HALO || y < HALO || y >= Ny - HALO) return;
+  const long long lat = (long long)b * 3 * p.plane;
+  double m[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const long long o = lat + c * p.plane + i;
+    const double vh = vz ? 0.0 : d.vel[o];
+    m[c] = d.phi[o] + d.alpha * vh;
+    if (d.use_acc) m[c] = m[c] + d.beta * d.acc[o];
+  }
+  CM<double>::project_field(m);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) d.phi_out[lat + c * p.plane + i] = m[c];
 }
 
 __global__ void __launch_bounds__(256) demag_rho_kernel(const __grid_constant__ DemagStepArgs A) {
@@ -273,10 +310,10 @@ __global__ void __launch_bounds__(DBX* DBY) demag_kick_kernel(const __grid_const
       G[1] += d.g * (p.i12h * Dyn<double>(T, 3));
       const double gn = (G[0] * n[0] + G[1] * n[1]) + G[2] * n[2];
       const double a[3] = {gn * n[0] - G[0], gn * n[1] - G[1], gn * n[2] - G[2]};
-      double e, q;
+      double e = 0.0, q = 0.0;
       const EdgeW w(gx, gy, Nx, Ny);
-      Th::densities(T, p, Bz, w, e, q);
-      {  // + g x bond density of psi (site form, halo weights R3)
+      if (d.advance != 2) Th::densities(T, p, Bz, w, e, q);
+      if (d.advance != 2) {  // + g x bond density of psi (site form, halo weights R3)
         const int ks[4] = {1, -1, 2, -2};
         double sA = 0.0, sB = 0.0;
 #pragma unroll
@@ -290,7 +327,7 @@ __global__ void __launch_bounds__(DBX* DBY) demag_kick_kernel(const __grid_const
       s0 = e;
       s1 = q;
       const long long o = (long long)gy * Nx + gx;
-      if (d.advance) {
+      if (d.advance == 1) {
         double u[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) u[c] = d.vel[lat + c * p.plane + o] + p.hdt * a[c];
@@ -316,12 +353,59 @@ __global__ void __launch_bounds__(DBX* DBY) demag_kick_kernel(const __grid_const
     }
   }
   __syncthreads();
-  if (tid < DTY && y0 + tid < Ny) {
+  if (d.advance != 2 && tid < DTY && y0 + tid < Ny) {
     const long long po = ((long long)b * Ny + (y0 + tid)) * p.nseg + blockIdx.x;
     d.part_e[po] = red[0][tid][0] + red[0][tid][1];
     d.part_q[po] = red[1][tid][0] + red[1][tid][1];
-    if (d.advance) d.part_ke[po] = red[2][tid][0] + red[2][tid][1];
+    if (d.advance == 1) d.part_ke[po] = red[2][tid][0] + red[2][tid][1];
   }
+}
+
+// RK4 combine (the oracle's expressions): phi' = R((phi + dt vh) + dt^2/6 ((a1 + a2)
+// + a3)), u = vh + dt/6 ((a1 + 2 a2) + (2 a3 + a4)), v' = u - (u.phi') phi', KE partial sums
+__global__ void __launch_bounds__(DBX* DBY) demag_combine_kernel(const __grid_constant__ DemagStepArgs A) {
+  const FlowArgs<double>& p = A.p;
+  const DemagArgs& d = A.d;
+  __shared__ double red[DTY][DBX / 32];
+  const int Nx = p.Nx, Ny = p.Ny;
+  const int b = blockIdx.z, x0 = blockIdx.x * DTX, y0 = blockIdx.y * DTY;
+  const long long lat = (long long)b * 3 * p.plane;
+  const int tid = threadIdx.y * DBX + threadIdx.x;
+  const bool vz = d.state[b].v_is_zero != 0;
+  const int gx = x0 + threadIdx.x;
+  const int warp_in_row = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll 2
+  for (int r = 0; r < DTY / DBY; ++r) {
+    const int ly = r * DBY + threadIdx.y, gy = y0 + ly;
+    double s0 = 0.0;
+    if (gx >= HALO && gx < Nx - HALO && gy >= HALO && gy < Ny - HALO) {
+      const long long o = (long long)gy * Nx + gx;
+      double f[3], u[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const long long oc = lat + c * p.plane + o;
+        const double vh = vz ? 0.0 : d.vel[oc];
+        const double A1 = d.a1[oc], A2 = d.a2[oc], A3 = d.a3[oc], A4 = d.a4[oc];
+        f[c] = (d.phi[oc] + p.dt * vh) + p.sdt2 * ((A1 + A2) + A3);
+        u[c] = vh + p.sdt * ((A1 + 2.0 * A2) + (2.0 * A3 + A4));
+      }
+      CM<double>::project_field(f);
+      CM<double>::project_velocity(u, f);
+      double v2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        d.phi_out[lat + c * p.plane + o] = f[c];
+        d.vel_out[lat + c * p.plane + o] = u[c];
+        v2 += u[c] * u[c];
+      }
+      s0 = 0.5 * v2;
+    }
+    s0 = warp_tree(s0);
+    if (lane == 0) red[ly][warp_in_row] = s0;
+  }
+  __syncthreads();
+  if (tid < DTY && y0 + tid < Ny)
+    d.part_ke[((long long)b * Ny + (y0 + tid)) * p.nseg + blockIdx.x] = red[tid][0] + red[tid][1];
 }
 
 }  // namespace ss

@@ -37,11 +37,12 @@ def _dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
 
 
-def _run(w, checkpoints, cycles, ftol, etol):
+def _run(w, checkpoints, cycles, ftol, etol, integrator="verlet"):
     ss = _ss()
-    s = ss.solver_for(w, integrator=ss.VERLET, demag_cycles=cycles)
+    s = ss.solver_for(w, integrator=ss.VERLET if integrator == "verlet" else ss.RK4,
+                      demag_cycles=cycles)
     s.set_fields(_dev(w.fields))
-    fl = oracle.Flow(_model(w), w.dt, integrator="verlet")
+    fl = oracle.Flow(_model(w), w.dt, integrator=integrator)
     fl.set_fields(w.fields[0])
     f0 = _floor(fl.m, w.fields[0], fl.energy)
     assert abs(s.energy()[0] - fl.energy) <= etol * f0
@@ -81,6 +82,21 @@ def test_demag_verlet_parity_on_a_ragged_lattice(dmi):
     assert np.abs(psi).max() > 1e-2                      # the term is not negligible here
 
 
+@pytest.mark.parametrize("dmi", [None, "neel"])
+def test_demag_rk4_parity_one_solve_per_stage(dmi):
+    # the paper's integrator with the demagnetising field: four Poisson solves per
+    # step (stage fields 2, 3, 4 and the new field), 146 x 130 unknowns (odd multigrid levels)
+    w = W.cm_single(N=150, K=0.1)
+    f = w.fields[:, :, :134, :].copy()
+    f[:, :, ~W.interior_mask(150, 134)] = np.array([0.0, 0.0, 1.0])[None, :, None]
+    w.fields, w.Ny = f, 134
+    w.demag = 0.8
+    if dmi:
+        w.dmi = W.DMI_NEEL
+    s, fl, _ = _run(w, (1, 2, 5, 10, 20, 50), cycles=24, ftol=1e-10, etol=1e-9, integrator="rk4")
+    assert s.schedule() != "resident-cluster" and len(fl.arrests()) >= 1
+
+
 def test_default_cycle_count_tracks_the_exact_solve_to_1e7():
     w = W.cm_single(N=128)
     w.demag = 1.0
@@ -93,10 +109,7 @@ def test_default_cycle_count_tracks_the_exact_solve_to_1e7():
 def test_demag_zero_coupling_equals_plain_verlet_and_unsupported_combinations():
     ss = _ss()
     w = W.cm_single(N=64)
-    with pytest.raises(ss.SSError) as e:
-        w.demag = 0.5
-        ss.solver_for(w)                                 # RK4 + demag
-    assert e.value.code == ss.ERR_UNSUPPORTED
+    w.demag = 0.5
     with pytest.raises(ss.SSError) as e:
         ss.solver_for(w, integrator=ss.VERLET, dtype=ss.F32)
     assert e.value.code == ss.ERR_UNSUPPORTED
