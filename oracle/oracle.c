@@ -23,6 +23,10 @@
  *   cm/ah gradients brute-force central differences of the bond-form energy (8x8)
  *   charges         integer degree of seeded ansaetze; unit flux of a vortex
  *   flow            RK4 order on AH; |n|=1, v.n=0; arrest invariants; Bogomolny bound
+ *   demagnetisation the CG Poisson solve inverts the pinned eq. (2) operator; 4th-order convergence
+ *                   to an analytic potential; divergence-free textures carry no field; E_d > 0 and
+ *                   E_d = -(g/2) h^2 sum psi rho; brute-force derivative of the plain energy with its
+ *                   own solve per evaluation; E_d(Neel) >> E_d(Bloch)
  *   baby Skyrme     brute-force gradient (12x12, radius-4 exact gradient), plain == site form,
  *                   vacuum, closed-form E4 / E0 of the hedgehog (1-D quadrature), Belavin-Polyakov
  *                   lump E2 = 4 pi, Derrick scaling and the virial E4 = E0 at the relaxed minimum
