@@ -31,7 +31,7 @@ namespace ss {
 
 constexpr int MGX = 32, MGY = 8;          // thread block of the multigrid kernels
 constexpr int MG_COARSE_MAX = 8;          // coarsen until both sizes are <= 8 (or one reaches 2)
-constexpr int MG_COARSE_SWEEPS = 100;  // spectral radius <= 0.96 on 8 x 8: residual x 0.02
+constexpr int MG_COARSE_SWEEPS = 40;       // measured: 40 sweeps keep the V-cycle at 0.27, 20 do not
 constexpr double MG_OMEGA = 10.0 / 13.0;  // 1 - 28 w/60 = -(1 - 128 w/60)
 
 // A level holds nx x ny unknowns inside a zero halo of width 2: arrays [batch][ny+4][nx+4].
