@@ -136,6 +136,10 @@ struct KernelNode {
   std::vector<unsigned char> args;  // the single by-value argument struct
   const char* name;
 };
+inline void set_args(KernelNode& n, const void* a, size_t bytes) {
+  n.args.resize(bytes);
+  memcpy(n.args.data(), a, bytes);
+}
 
 }  // namespace
 
@@ -325,7 +329,7 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   n.grid = dim3(s->L.nseg, (NC + s->cps[kind] - 1) / s->cps[kind], s->batch);
   n.block = dim3(flow_threads(s->ktheory, s->dtype, kind), 1, 1);
   n.smem = (size_t)flow_smem(s->ktheory, s->dtype, kind);
-  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  set_args(n, &a, sizeof(a));
   n.name = kind == KX   ? "flow_x_grad_energy_charge_stage2"
            : kind == KY ? "flow_y_stage34_combine_project_ke"
                         : "flow_v_verlet_step_energy_charge_ke";
@@ -380,7 +384,7 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
   n.grid = dim3((s->Nx + BTX - 1) / BTX, (s->Ny + BTY - 1) / BTY, s->batch);
   n.block = dim3(BBX, BBY, 1);
   n.smem = sizeof(BsSmem<real>);
-  n.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  set_args(n, &a, sizeof(a));
   static const char* names[4] = {"bs_stage1_grad_energy_charge", "bs_stage2", "bs_stage3",
                                  "bs_stage4_combine_project_ke"};
   n.name = names[stage - 1];
@@ -395,7 +399,7 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
 KernelNode mg_node(void* func, const MgArgs& m, dim3 grid, dim3 block, size_t smem, const char* name) {
   KernelNode n;
   n.func = func; n.grid = grid; n.block = block; n.smem = smem; n.name = name;
-  n.args.assign((const unsigned char*)&m, (const unsigned char*)&m + sizeof(m));
+  set_args(n, &m, sizeof(m));
   return n;
 }
 void add_vcycle(const ss_solver* s, size_t l, std::vector<KernelNode>& out) {
@@ -469,7 +473,7 @@ void make_demag_step(const ss_solver* s, int cur, std::vector<KernelNode>& st,
   auto node = [&](void* f, const DemagStepArgs& x, dim3 grid, dim3 block, const char* name) {
     KernelNode n;
     n.func = f; n.grid = grid; n.block = block; n.smem = 0; n.name = name;
-    n.args.assign((const unsigned char*)&x, (const unsigned char*)&x + sizeof(x));
+    set_args(n, &x, sizeof(x));
     return n;
   };
   if (s->integrator == SS_RK4) {  // one Poisson solve per stage field (ss_demag.cuh header)
@@ -560,7 +564,7 @@ void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>&
   r.grid = dim3((s->Ny + 7) / 8, s->batch, 1);
   r.block = dim3(256, 1, 1);
   r.smem = 0;
-  r.args.assign((unsigned char*)&a, (unsigned char*)&a + sizeof(a));
+  set_args(r, &a, sizeof(a));
   r.name = "row_reduce";
   out.push_back(r);
   KernelNode f = r;
