@@ -153,7 +153,8 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
 
 /* Enqueue k flow steps (asynchronous; no host synchronisation, the arrest of eq. 4 is
  * decided on the device; the steps are CUDA-graph replays, 8 steps per graph launch plus
- * single-step graphs for the remainder).  One step = RK4 stages 2-4 + update + projection, then the
+ * single-step graphs for the remainder; steps of more than 64 kernels -- demagnetisation -- are
+ * replayed one step per graph launch).  One step = RK4 stages 2-4 + update + projection, then the
  * stencil pass on the new field (a, E, Q) and the arrest decision.
  * Small lattices (fp64 chiral magnet, SS_RK4, Nx a multiple of 32, the whole state within the
  * shared memory of one thread-block cluster per lattice, e.g. 64 x 64 ... 128 x 128) take all k

@@ -851,7 +851,9 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (rc != SS_OK) { ss_destroy(s); return rc; }
     }
   }
-  if (!(s->flags & SS_FLAG_NO_GRAPH)) {  // MULTI steps chained in one graph: fewer launches, no inter-graph gaps
+  // MULTI steps chained in one graph: fewer launches, no inter-graph gaps.  A step that is already
+  // hundreds of nodes long (demagnetisation: ~50 nodes per V-cycle) gains nothing from chaining.
+  if (!(s->flags & SS_FLAG_NO_GRAPH) && s->step_nodes[0].size() <= 64) {
     for (int cur = 0; cur < 2; ++cur) {
       std::vector<KernelNode> chain;
       for (int i = 0; i < MULTI; ++i) {
@@ -974,7 +976,7 @@ int ss_step(ss_solver* s, int64_t k) {
     if (s->flags & SS_FLAG_NO_GRAPH) {
       int rc = launch_nodes(s, s->step_nodes[s->cur]);
       if (rc != SS_OK) return rc;
-    } else if (k - it >= MULTI) {  // MULTI is even: the parity is unchanged afterwards
+    } else if (k - it >= MULTI && s->multi_exec[s->cur]) {  // MULTI is even: same parity afterwards
       CK(cudaGraphLaunch(s->multi_exec[s->cur], s->stream));
       s->launches += (int64_t)MULTI * (int64_t)s->step_nodes[s->cur].size();
       s->steps_done += MULTI;
