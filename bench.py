@@ -247,6 +247,7 @@ KERNEL_UNITS = {
     "bs_stage3": 4,                       # reads phi, v, a1         -> writes a3
     "bs_stage4_combine_project_ke": 7,    # reads phi, v, a1, a2, a3 -> writes phi', v'
     "bs_stage1_grad_energy_charge": 2,    # reads phi'               -> writes a1 (+ E, Q partials)
+    "bs_verlet_step_energy_charge_ke": 6, # reads phi, v, a          -> writes phi', v', a'
     # demagnetisation (csrc/ss_demag.cuh), units of C*R with C = 3: drift reads phi, v, a, writes
     # phi', w; kick reads phi', w, psi, writes a', v'; rho and the multigrid kernels move single
     # planes and are reported by their time only

@@ -15,8 +15,8 @@
  *       SS_THEORY_ABELIAN_HIGGS  phi in C, A in R^2: 1/2|D phi|^2 + 1/2 (curl A)^2
  *                                + (lambda/8)(1-|phi|^2)^2   (DESIGN R1-R3, R9),
  *       SS_THEORY_BABY_SKYRME    m in S^2: 1/2|grad m|^2 + (kappa^2/2)|d1 m x d2 m|^2 + V(m)
- *                                (DESIGN R18; SS_RK4 only, C = 3, charge =
- *                                degree as for the chiral magnet);
+ *                                (DESIGN R18; C = 3, charge = degree as for
+ *                                the chiral magnet);
  *   - the arrested Newton flow phi'' = -grad E_h (eq. 3) integrated with
  *     classical RK4, the unit-length projection applied in every stage
  *     (PAPER.md:129+154), the velocity set to zero whenever E_h rises (eq. 4);

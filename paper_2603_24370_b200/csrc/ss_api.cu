@@ -349,7 +349,8 @@ void* bs_func(int stage) {
     case 1: return (void*)bs_stage_kernel<real, 1>;
     case 2: return (void*)bs_stage_kernel<real, 2>;
     case 3: return (void*)bs_stage_kernel<real, 3>;
-    default: return (void*)bs_stage_kernel<real, 4>;
+    case 4: return (void*)bs_stage_kernel<real, 4>;
+    default: return (void*)bs_stage_kernel<real, 5>;
   }
 }
 template <typename real>
@@ -363,6 +364,10 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
   a.vel = (const real*)s->vel(cur);
   a.aprev = stage == 3 ? (const real*)s->acc(0) : (const real*)s->acc(1);  // stage 4: a2
   a.aout = (real*)s->acc(stage == 1 ? 0 : stage == 2 ? 1 : 2);
+  if (s->integrator == SS_VERLET) {  // stage 5 steps cur -> cur ^ 1; stage 1 evaluates buffer cur
+    a.aprev = (const real*)s->acc(cur);
+    a.aout = (real*)s->acc(stage == 1 ? cur : cur ^ 1);
+  }
   a.a1 = (const real*)s->acc(0);
   a.a3 = (const real*)s->acc(2);
   a.phi_out = (real*)s->phi(cur ^ 1);
@@ -373,7 +378,7 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
   // stage fields: phi2 = R(phi + dt/2 v), phi3 = R((phi + dt/2 v) + dt^2/4 a1),
   // phi4 = R((phi + dt v) + dt^2/2 a2)
   a.alpha = stage == 4 ? k.dt : k.hdt;
-  a.beta = stage == 3 ? k.qdt2 : k.hdt2;
+  a.beta = stage == 5 ? k.hdt : (stage == 3 ? k.qdt2 : k.hdt2);
   a.dt = k.dt; a.sdt2 = k.sdt2; a.sdt = k.sdt;
   a.i12h = k.i12h; a.i12h2 = k.i12h2;
   a.lap0 = k.lap0; a.lap1 = k.lap1; a.lap2 = k.lap2;
@@ -385,8 +390,8 @@ KernelNode make_bs_node(const ss_solver* s, int stage, int cur) {
   n.block = dim3(BBX, BBY, 1);
   n.smem = sizeof(BsSmem<real>);
   set_args(n, &a, sizeof(a));
-  static const char* names[4] = {"bs_stage1_grad_energy_charge", "bs_stage2", "bs_stage3",
-                                 "bs_stage4_combine_project_ke"};
+  static const char* names[5] = {"bs_stage1_grad_energy_charge", "bs_stage2", "bs_stage3",
+                                 "bs_stage4_combine_project_ke", "bs_verlet_step_energy_charge_ke"};
   n.name = names[stage - 1];
   return n;
 }
@@ -702,8 +707,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
   if (p->flags & ~(SS_FLAG_NO_GRAPH | SS_FLAG_NO_RESIDENT)) return SS_ERR_ARG;
-  if (theory == SS_THEORY_BABY_SKYRME && (p->integrator != SS_RK4 || p->dmi_d))
-    return SS_ERR_UNSUPPORTED;  // the baby-Skyrme kernels exist for the RK4 step only
+  if (theory == SS_THEORY_BABY_SKYRME && p->dmi_d) return SS_ERR_UNSUPPORTED;
   if (!std::isfinite(p->demag) || p->demag < 0.0 || p->demag_cycles < 0) return SS_ERR_ARG;
   if (p->demag != 0.0 && theory == SS_THEORY_CHIRAL_MAGNET && p->dtype != SS_F64)
     return SS_ERR_UNSUPPORTED;  // demagnetisation: fp64 only
@@ -794,7 +798,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
   }
   if (s->ktheory == kBS) {
-    for (int stage = 1; stage <= 4; ++stage) {
+    for (int stage = 1; stage <= 5; ++stage) {
       void* f = p->dtype == SS_F64 ? bs_func<double>(stage) : bs_func<float>(stage);
       const size_t smem = p->dtype == SS_F64 ? sizeof(BsSmem<double>) : sizeof(BsSmem<float>);
       e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -820,10 +824,14 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     if (s->demag != 0.0) {
       make_demag_step(s, cur, st, ev);
     } else if (s->ktheory == kBS) {
-      st.push_back(make_bs_node(s, 2, cur));
-      st.push_back(make_bs_node(s, 3, cur));
-      st.push_back(make_bs_node(s, 4, cur));
-      st.push_back(make_bs_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
+      if (s->integrator == SS_VERLET) {
+        st.push_back(make_bs_node(s, 5, cur));  // the whole step: phi', v', a', E, Q, KE
+      } else {
+        st.push_back(make_bs_node(s, 2, cur));
+        st.push_back(make_bs_node(s, 3, cur));
+        st.push_back(make_bs_node(s, 4, cur));
+        st.push_back(make_bs_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
+      }
       ev.push_back(make_bs_node(s, 1, cur));
     } else if (s->integrator == SS_VERLET) {
       KernelNode v, x0;

@@ -12,6 +12,9 @@
 //       STAGE 1: psi = phi; also site energy / degree densities -> row-segment partial sums
 //       STAGE 4: + RK4 combine, projections (PAPER.md:129+154), KE partial sums, writes the new
 //                (phi, v) into the other ping-pong buffer
+//       STAGE 5: the whole one-gradient-per-step (velocity Verlet, DESIGN R15) step: psi = phi_new
+//                = R(phi + dt (vh + dt/2 a)), a_new = -Pi G(phi_new), v_new = Pi(vh + dt/2 a +
+//                dt/2 a_new), e, q, KE partial sums; writes phi_new, v_new, a_new
 //
 // Algorithmic bytes: stage 2 reads phi, v, writes a2 (3 C R); stage 3 reads phi, v, a1, writes a3
 // (4); stage 4 reads phi, v, a1, a2, a3, writes phi', v' (7); stage 1 reads phi', writes a1 (2):
@@ -65,7 +68,7 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
   using Th = BS<real>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   BsSmem<real>& sm = *reinterpret_cast<BsSmem<real>*>(smem_raw);
-  __shared__ double red[2][BTY][BBX / 32];
+  __shared__ double red[3][BTY][BBX / 32];
 
   const int Nx = p.Nx, Ny = p.Ny;
   const int b = blockIdx.z;
@@ -101,7 +104,22 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
     for (int k = 0; k < NS1; ++k)
 #pragma unroll
       for (int c = 0; c < 3; ++c) m[k][c] = in[k] ? phi[c * p.plane + off[k]] : real(0);
-    if (STAGE > 1) {  // halo sites of every stage field are the frozen halo
+    if (STAGE == 5) {  // velocity Verlet (DESIGN R15): phi' = R(phi + dt (vh + dt/2 a))
+      real v[NS1][3], ap[NS1][3];
+#pragma unroll
+      for (int k = 0; k < NS1; ++k)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          v[k][c] = (inter[k] && !vz) ? vel[c * p.plane + off[k]] : real(0);
+          ap[k][c] = inter[k] ? aprev[c * p.plane + off[k]] : real(0);
+        }
+#pragma unroll
+      for (int k = 0; k < NS1; ++k) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) m[k][c] = m[k][c] + p.dt * (v[k][c] + p.beta * ap[k][c]);
+        if (inter[k]) Th::project_field(m[k]);
+      }
+    } else if (STAGE > 1) {  // halo sites of every stage field are the frozen halo
       if (!vz) {
         real v[NS1][3];
 #pragma unroll
@@ -179,7 +197,7 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
     const int ly = r * BBY + threadIdx.y;
     const int gy = y0 + ly;
     const bool active = interior(gx, gy);
-    double s0 = 0.0, s1 = 0.0;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
     if (active) {
       const int cx = threadIdx.x + BH, cy = ly + BH;
       auto T = [&](int c, int dy, int dx) -> real { return sm.m[c][cy + dy][cx + dx]; };
@@ -199,15 +217,33 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
       const real gn = (G[0] * m[0] + G[1] * m[1]) + G[2] * m[2];
       const real a[3] = {gn * m[0] - G[0], gn * m[1] - G[1], gn * m[2] - G[2]};
       const long long o = (long long)gy * Nx + gx;
-      if (STAGE < 4) {
+      if (STAGE != 4) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) p.aout[lat + c * p.plane + o] = a[c];
       }
-      if (STAGE == 1) {
+      if (STAGE == 1 || STAGE == 5) {
         real e, q;
         Th::densities(T, p, real(0), EdgeW(gx, gy, Nx, Ny), e, q);
         s0 = double(e);
         s1 = double(q);
+      }
+      if (STAGE == 5) {  // second half kick with the new acceleration, tangent projection, KE
+        real u[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const long long oc = c * p.plane + o;
+          const real vh = vz ? real(0) : vel[oc];
+          u[c] = (vh + p.beta * aprev[oc]) + p.beta * a[c];
+        }
+        Th::project_velocity(u, m);
+        real v2 = real(0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          p.phi_out[lat + c * p.plane + o] = m[c];
+          p.vel_out[lat + c * p.plane + o] = u[c];
+          v2 += u[c] * u[c];
+        }
+        s2 = 0.5 * double(v2);
       }
       if (STAGE == 4) {
         real f[3], u[3];
@@ -231,23 +267,26 @@ __global__ void __launch_bounds__(BBX* BBY, 2) bs_stage_kernel(const __grid_cons
         s0 = 0.5 * double(v2);
       }
     }
-    if (STAGE == 1 || STAGE == 4) {  // first five levels of the canonical tree (DESIGN R10)
+    if (STAGE == 1 || STAGE >= 4) {  // first five levels of the canonical tree (DESIGN R10)
       s0 = warp_tree(s0);
-      if (STAGE == 1) s1 = warp_tree(s1);
+      if (STAGE != 4) s1 = warp_tree(s1);
+      if (STAGE == 5) s2 = warp_tree(s2);
       if (lane == 0) {
         red[0][ly][warp_in_row] = s0;
-        if (STAGE == 1) red[1][ly][warp_in_row] = s1;
+        if (STAGE != 4) red[1][ly][warp_in_row] = s1;
+        if (STAGE == 5) red[2][ly][warp_in_row] = s2;
       }
     }
   }
-  if (STAGE == 1 || STAGE == 4) {
+  if (STAGE == 1 || STAGE >= 4) {
     __syncthreads();
     if (tid < BTY && y0 + tid < Ny) {
       const long long po = ((long long)b * Ny + (y0 + tid)) * p.nseg + blockIdx.x;
       static_assert(BBX / 32 == 2, "row segment = two warps");
-      if (STAGE == 1) {
+      if (STAGE != 4) {
         p.part_e[po] = red[0][tid][0] + red[0][tid][1];
         p.part_q[po] = red[1][tid][0] + red[1][tid][1];
+        if (STAGE == 5) p.part_ke[po] = red[2][tid][0] + red[2][tid][1];
       } else {
         p.part_ke[po] = red[0][tid][0] + red[0][tid][1];
       }

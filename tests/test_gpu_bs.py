@@ -38,13 +38,13 @@ def _ragged(w, Ny):
     return w
 
 
-def _run(w, checkpoints, flags=0):
+def _run(w, checkpoints, flags=0, integrator="rk4"):
     ss = _ss()
-    s = ss.solver_for(w, flags=flags)
+    s = ss.solver_for(w, flags=flags, integrator=ss.VERLET if integrator == "verlet" else ss.RK4)
     s.set_fields(_dev(w.fields))
     flows = []
     for b in range(w.batch):
-        fl = oracle.Flow(_model(w), w.dt)
+        fl = oracle.Flow(_model(w), w.dt, integrator=integrator)
         fl.set_fields(w.fields[b])
         flows.append(fl)
         f0 = _floor(fl.m, w.fields[b], fl.energy)
@@ -82,6 +82,16 @@ def test_bs_first_100_steps_on_a_ragged_lattice(pot, potN):
     assert float(((phi * phi).sum(1) - 1.0).abs().max()) < 1e-14
 
 
+@pytest.mark.parametrize("pot", [W.POT_STANDARD, W.POT_BROKEN])
+def test_bs_verlet_first_100_steps(pot):
+    # the one-gradient-per-step integrator (DESIGN R15) through the stage-5 tile kernel
+    w = _ragged(W.bs_single(N=150, pot=pot), 134)
+    s, flows = _run(w, (1, 2, 5, 10, 20, 50, 100), integrator="verlet")
+    assert len(flows[0].arrests()) >= 1
+    w = W.bs_single(N=96, count=2, batch=2, kappa=0.8, mu=0.7)
+    _run(w, (1, 5, 20), integrator="verlet")
+
+
 def test_bs_batched_multi_skyrmion_and_smallest_lattices():
     w = W.bs_single(N=140, count=3, batch=2, kappa=0.8, mu=0.7)
     s, flows = _run(w, (1, 2, 5, 10, 20, 50))
@@ -114,8 +124,9 @@ def test_bs_vacuum_graph_vs_direct_and_unsupported():
         outs.append((f.cpu(), v.cpu(), s.energy(), s.charge(), s.arrests(0)))
     assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
     assert outs[0][2:] == outs[1][2:]
+    w.dmi = W.DMI_NEEL
     with pytest.raises(ss.SSError) as e:
-        ss.solver_for(w, integrator=ss.VERLET)
+        ss.solver_for(w)                                  # no DMI table in this theory
     assert e.value.code == ss.ERR_UNSUPPORTED
     with pytest.raises(ss.SSError) as e:
         ss.Solver(ss.THEORY_BABY_SKYRME, 64, 64, 0.2, pot=7)
