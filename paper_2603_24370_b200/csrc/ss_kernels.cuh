@@ -6,16 +6,28 @@
 
 namespace ss {
 
-// In-thread aligned pairwise tree over m (power of two, <= 32) consecutive values.
-__device__ __forceinline__ double chunk_tree(const double* src, long long first, long long n, int m) {
-  double t[32];
-#pragma unroll 1
-  for (int i = 0; i < m; ++i) t[i] = (first + i < n) ? src[first + i] : 0.0;
-#pragma unroll 1
-  for (int s = m; s > 1; s >>= 1)
-#pragma unroll 1
+// In-thread aligned pairwise tree over m (power of two, <= 32) consecutive values: all loads are
+// issued first, the tree runs in registers (one instance per m).
+template <int M>
+__device__ __forceinline__ double chunk_tree_m(const double* src, long long first, long long n) {
+  double t[M];
+#pragma unroll
+  for (int i = 0; i < M; ++i) t[i] = (first + i < n) ? src[first + i] : 0.0;
+#pragma unroll
+  for (int s = M; s > 1; s >>= 1)
+#pragma unroll
     for (int i = 0; i < s / 2; ++i) t[i] = t[2 * i] + t[2 * i + 1];
   return t[0];
+}
+__device__ __forceinline__ double chunk_tree(const double* src, long long first, long long n, int m) {
+  switch (m) {
+    case 1: return chunk_tree_m<1>(src, first, n);
+    case 2: return chunk_tree_m<2>(src, first, n);
+    case 4: return chunk_tree_m<4>(src, first, n);
+    case 8: return chunk_tree_m<8>(src, first, n);
+    case 16: return chunk_tree_m<16>(src, first, n);
+    default: return chunk_tree_m<32>(src, first, n);
+  }
 }
 
 // One warp per lattice row: finishes the x-tree over the nseg segment partials of that row.
