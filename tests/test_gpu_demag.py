@@ -137,3 +137,30 @@ def test_paper_usage_example_shape_antiskyrmion_with_demag():
     s, fl, _ = _run(w, (5, 10, 15, 20), cycles=24, ftol=1e-10, etol=1e-9)
     assert abs(s.charge()[0] - 1.0) < 5e-3
     assert fl.energy < oracle.energy_charge(_model(w), w.fields[0])[0]
+
+
+def test_batched_demag_with_per_lattice_B():
+    # three lattices with their own B and their own potential psi (blockIdx.z through every
+    # multigrid kernel, one coarsest-level CTA per lattice)
+    ss = _ss()
+    w = W.cm_sweep(batch=3, N=80)
+    w.demag, w.dmi = 0.7, W.DMI_NEEL
+    s = ss.solver_for(w, integrator=ss.VERLET, demag_cycles=24)
+    s.set_fields(_dev(w.fields))
+    flows = []
+    for b in range(w.batch):
+        m = oracle.model(oracle.CM, w.Nx, w.Ny, w.h, kappa=w.kappa, B=float(w.B_batch[b]), K=w.K,
+                         dmi=w.dmi, demag=w.demag)
+        fl = oracle.Flow(m, w.dt, integrator="verlet")
+        fl.set_fields(w.fields[b])
+        flows.append(fl)
+    for k in (1, 9, 20):
+        s.step(k)
+        phi, vel = s.get_fields()
+        E = s.energy()
+        for b, fl in enumerate(flows):
+            fl.step(k)
+            ophi, _ = fl.get_fields()
+            assert np.abs(phi[b].cpu().numpy() - ophi).max() <= 1e-10, (k, b)
+            assert abs(E[b] - fl.energy) <= 1e-9 * _floor(fl.m, ophi, fl.energy), (k, b)
+            assert s.arrests(b)[0] == fl.arrests()
