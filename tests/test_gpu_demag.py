@@ -164,3 +164,36 @@ def test_batched_demag_with_per_lattice_B():
             assert np.abs(phi[b].cpu().numpy() - ophi).max() <= 1e-10, (k, b)
             assert abs(E[b] - fl.energy) <= 1e-9 * _floor(fl.m, ophi, fl.energy), (k, b)
             assert s.arrests(b)[0] == fl.arrests()
+
+
+def test_demag_bench_size_properties():
+    """bench.py's demagnetisation workload (2048 x 2048, 64 skyrmions, Neel DMI, g = 1) in the
+    launch configuration it times (default 8 V-cycles, CUDA graph).  The oracle's exact CG solve
+    is minutes per step at this size, so this checks what holds at any size: E never rises except
+    at the steps the device logged, |n| = 1, v.n = 0, the halo is frozen, and the default cycle
+    count tracks a 24-cycle run of the same lattice to 1e-6."""
+    ss = _ss()
+    w = W.cm_demag_bench()
+    x = _dev(w.fields)
+    a = ss.solver_for(w, integrator=ss.VERLET)
+    b = ss.solver_for(w, integrator=ss.VERLET, demag_cycles=24)
+    for s in (a, b):
+        s.set_fields(x)
+    E = [a.energy()[0]]
+    for _ in range(30):
+        a.step(1)
+        E.append(a.energy()[0])
+    arrests = set(a.arrests(0)[0])
+    for n in range(1, len(E)):
+        assert (E[n] > E[n - 1]) == (n in arrests), n
+    assert E[-1] < E[0] and a.status()["steps"] == 30
+    b.step(30)
+    fa, va = a.get_fields()
+    fb, _ = b.get_fields()
+    assert float((fa - fb).abs().max()) < 1e-6
+    assert abs(a.energy()[0] - b.energy()[0]) < 1e-6 * abs(b.energy()[0])
+    mask = torch.from_numpy(~W.interior_mask(w.Nx, w.Ny)).to("cuda:0")
+    assert torch.equal(fa[0][:, mask], x[0][:, mask])
+    assert float(((fa[0] * fa[0]).sum(0)[~mask] - 1.0).abs().max()) < 1e-14
+    if not a.status()["n_arrests"][0] or 30 not in arrests:
+        assert float((fa[0] * va[0]).sum(0)[~mask].abs().max()) < 1e-12
