@@ -26,7 +26,6 @@ import argparse
 import json
 import os
 import sys
-import threading
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -83,50 +82,55 @@ def peaks():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML during the timed region."""
+class ClockSampler:
+    """SM clock, power and throttle reasons through NVML during a timed region.
 
-    def __init__(self, index, period=0.002):
-        super().__init__(daemon=True)
+    No thread: the caller records the region's end event and then `wait(event)` polls that event
+    from the main thread, taking one NVML sample (about 3 us of host time) every `period` seconds
+    until the event has completed, so even a 15 ms region carries >= 10 samples and every sample
+    lies inside the region."""
+
+    def __init__(self, index, period=0.0005):
         self.index, self.period = index, period
         self.samples, self.power, self.reasons, self.max_mhz = [], [], set(), None
-        self._stop_evt = threading.Event()
         try:
             import pynvml
             pynvml.nvmlInit()
-            self.nv = pynvml
-            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
-            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            nv = self.nv = pynvml
+            self.h = nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+            self.names = {
+                nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+                nv.nvmlClocksThrottleReasonApplicationsClocksSetting: "applications_clocks",
+            }
         except Exception:
             self.nv = None
 
-    def run(self):
+    def sample(self):
         if self.nv is None:
             return
         nv = self.nv
-        names = {
-            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
-            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
-            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
-            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
-            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
-            nv.nvmlClocksThrottleReasonApplicationsClocksSetting: "applications_clocks",
-        }
-        while not self._stop_evt.is_set():
-            try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
-                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) * 1e-3)
-                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, nm in names.items():
-                    if r & bit:
-                        self.reasons.add(nm)
-            except Exception:
-                pass
-            self._stop_evt.wait(self.period)
+        try:
+            self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+            self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) * 1e-3)
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            for bit, nm in self.names.items():
+                if r & bit:
+                    self.reasons.add(nm)
+        except Exception:
+            pass
+
+    def wait(self, event):
+        """Sample until `event` (recorded at the end of the timed region) has completed."""
+        while not event.query():
+            self.sample()
+            time.sleep(self.period)
 
     def stop(self):
-        self._stop_evt.set()
-        self.join(timeout=2.0)
         s = sorted(self.samples)
         pw = sorted(self.power)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
@@ -370,11 +374,11 @@ def run_ours(args):
     barrier()
     n0 = s.launch_count()
     sampler = ClockSampler(nvml_index(torch, dev))
-    sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(s.stream)
     s.step(args.steps)
     e1.record(s.stream)
+    sampler.wait(e1)
     barrier()
     clocks = sampler.stop()
     launches = s.launch_count() - n0
@@ -395,11 +399,11 @@ def run_ours(args):
         n = (n + 7) // 8 * 8
         barrier()
         sam2 = ClockSampler(nvml_index(torch, dev), period=0.01)
-        sam2.start()
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         f0.record(s.stream)
         s.step(n)
         f1.record(s.stream)
+        sam2.wait(f1)
         barrier()
         c2 = sam2.stop()
         ms2 = max_over_ranks([f0.elapsed_time(f1)], dist if world > 1 else None, dev)[0]
