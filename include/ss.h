@@ -78,8 +78,11 @@ enum { SS_RK4 = 0, SS_VERLET = 1 };
 /* ss_params.flags (debugging aid, not part of the method) */
 enum { SS_FLAG_NO_GRAPH = 1,   /* launch the step's kernels one by one instead of replaying the
                                   per-step CUDA graphs; results are bitwise identical */
-       SS_FLAG_NO_RESIDENT = 2 /* never use the resident-cluster schedule (see ss_step); results
-                                  are bitwise identical */ };
+       SS_FLAG_NO_RESIDENT = 2,/* never use the resident-cluster schedule (see ss_step); results
+                                  are bitwise identical */
+       SS_FLAG_NO_SLABS = 4    /* never split the RK4 step's two kernels into row slabs that
+                                  overlap inside the graph (see ss_step); results are bitwise
+                                  identical */ };
 
 typedef struct {
   int dtype;               /* SS_F64 | SS_F32: field storage and per-site arithmetic;       */
@@ -159,7 +162,11 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
  * Small lattices (fp64 chiral magnet, SS_RK4, Nx a multiple of 32, the whole state within the
  * shared memory of one thread-block cluster per lattice, e.g. 64 x 64 ... 128 x 128) take all k
  * steps in ONE launch with the state resident in shared memory; fields, E, Q, KE and the arrest
- * log are bitwise identical to the general schedule. */
+ * log are bitwise identical to the general schedule.
+ * Large single lattices (SS_RK4, at least three waves of CTAs and eight row segments, e.g.
+ * 2048 x 2048 Abelian Higgs, 4096 x 4096) have the step's two flow kernels split into four row
+ * slabs each, joined in the graph by the data dependencies only, so that the second kernel
+ * starts on the rows the first has finished; again bitwise identical (SS_FLAG_NO_SLABS). */
 int ss_step(ss_solver* s, int64_t k);
 
 /* Scalar read-outs: synchronise the stream, then fill HOST arrays of length batch.

@@ -135,6 +135,7 @@ struct KernelNode {
   size_t smem;
   std::vector<unsigned char> args;  // the single by-value argument struct
   const char* name;
+  std::vector<int> back;            // graph edges: waits for nodes i - back[k]; empty = {1}
 };
 inline void set_args(KernelNode& n, const void* a, size_t bytes) {
   n.args.resize(bytes);
@@ -163,6 +164,8 @@ struct ss_solver {
   double dmi[6];  // (d_x, d_y) of the table
   int64_t steps_done, launches;
   std::vector<KernelNode> step_nodes[2];  // per parity: Y, X (or V), row_reduce, finalize
+  std::vector<KernelNode> prof_nodes[2];  // slab schedule: the unsplit Y, X, reductions (profiling)
+  int slabs;                              // > 1: row-slab pipelined RK4 step
   std::vector<KernelNode> eval_nodes[2];  // X, row_reduce, finalize(advance = 0)
   cudaGraphExec_t step_exec[2];   // one flow step, per ping-pong parity
   cudaGraphExec_t multi_exec[2];  // MULTI consecutive steps in one graph (k steps per launch)
@@ -303,7 +306,7 @@ void fill_constants(const ss_solver* s, FlowArgs<real>& a) {
 // kernel X (kind KX) evaluates the state in buffer `in`; kernels Y and V advance `in` -> `in ^ 1`
 // (V also a: acc(in) -> acc(in ^ 1))
 template <typename real>
-bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
+bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out, int seg0, int nsegy) {
   FlowArgs<real> a;
   memset(&a, 0, sizeof(a));
   if (!make_tmap(s, s->phi(in), &a.tm[0]) || !make_tmap(s, s->vel(in), &a.tm[1]) ||
@@ -323,10 +326,11 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   a.Bb = (const double*)(s->ws + s->L.off_bb);
   fill_constants(s, a);
   a.cps = s->cps[kind];
+  a.seg0 = seg0;  // this launch covers y-segments [seg0, seg0 + nsegy); nsegy = 0: all of them
   KernelNode n;
   n.func = flow_func(s->ktheory, s->dtype, kind);
   const int NC = (s->Ny + FR - 1) / FR;
-  n.grid = dim3(s->L.nseg, (NC + s->cps[kind] - 1) / s->cps[kind], s->batch);
+  n.grid = dim3(s->L.nseg, nsegy > 0 ? nsegy : (NC + s->cps[kind] - 1) / s->cps[kind], s->batch);
   n.block = dim3(flow_threads(s->ktheory, s->dtype, kind), 1, 1);
   n.smem = (size_t)flow_smem(s->ktheory, s->dtype, kind);
   set_args(n, &a, sizeof(a));
@@ -336,9 +340,9 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
   *out = n;
   return true;
 }
-bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out) {
-  return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out)
-                            : make_flow_node<float>(s, kind, in, out);
+bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out, int seg0 = 0, int nsegy = 0) {
+  return s->dtype == SS_F64 ? make_flow_node<double>(s, kind, in, out, seg0, nsegy)
+                            : make_flow_node<float>(s, kind, in, out, seg0, nsegy);
 }
 
 // baby Skyrme: one tile kernel per RK4 stage (ss_bs.cuh); stage 1 evaluates buffer `cur`,
@@ -552,6 +556,30 @@ int choose_cps(int nstrips, int Ny, int batch, int slots) {
   return best_cps;
 }
 
+// Row-slab pipelining of the RK4 step (ss_create): one lattice, tall enough for SLABS slabs of at
+// least two segments each, and at least three waves of CTAs -- below that the split only costs
+// (cm 1024^2: 0.084 vs 0.079 ms; 256 lattices of 256^2 split by lattice: -0.3 %, not built).
+// With the tail of Y filled by X the best segment is shorter than choose_cps's: about four
+// waves of CTAs in all, not below 12 chunks (measured: cm 4096^2 fp64 flat over 22..38 chunks,
+// fp32 best at 24, Abelian Higgs 2048^2 best at 14..16).
+constexpr int SLABS = 4;
+void plan_slabs(ss_solver* s, int user_cps, int slots) {
+  s->slabs = 0;
+  if (s->integrator != SS_RK4 || s->ktheory == kBS || s->demag != 0.0 || s->batch != 1) return;
+  if (s->flags & SS_FLAG_NO_SLABS) return;
+  const int NC = (s->Ny + FR - 1) / FR;
+  int cps = user_cps;
+  if (cps <= 0) {
+    const int segs = (4 * slots + s->L.nseg - 1) / s->L.nseg;
+    cps = (NC + segs - 1) / (segs > 0 ? segs : 1);
+    if (cps < 12) cps = 12;
+  }
+  const int nsy = (NC + cps - 1) / cps;
+  if (nsy < 2 * SLABS || (long long)nsy * s->L.nseg < 3LL * slots) return;
+  s->slabs = SLABS;
+  s->cps[KX] = s->cps[KY] = cps;
+}
+
 void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>& out) {
   ReduceArgs a;
   memset(&a, 0, sizeof(a));
@@ -592,8 +620,7 @@ int launch_nodes(ss_solver* s, std::vector<KernelNode>& nodes) {
 int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* exec) {
   cudaGraph_t g;
   CK(cudaGraphCreate(&g, 0));
-  cudaGraphNode_t prev{};
-  bool have_prev = false;
+  std::vector<cudaGraphNode_t> made;
   for (auto& n : nodes) {
     cudaKernelNodeParams kp;
     memset(&kp, 0, sizeof(kp));
@@ -604,10 +631,17 @@ int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* e
     kp.sharedMemBytes = (unsigned)n.smem;
     kp.kernelParams = params;
     cudaGraphNode_t node;
-    cudaError_t e = cudaGraphAddKernelNode(&node, g, have_prev ? &prev : nullptr, have_prev ? 1 : 0, &kp);
+    std::vector<cudaGraphNode_t> deps;
+    const int i = (int)made.size();
+    if (n.back.empty()) {
+      if (i > 0) deps.push_back(made[i - 1]);
+    } else {
+      for (int bk : n.back)
+        if (i - bk >= 0) deps.push_back(made[i - bk]);
+    }
+    cudaError_t e = cudaGraphAddKernelNode(&node, g, deps.data(), deps.size(), &kp);
     if (!cuda_ok(e, "cudaGraphAddKernelNode")) { cudaGraphDestroy(g); return SS_ERR_CUDA; }
-    prev = node;
-    have_prev = true;
+    made.push_back(node);
   }
   cudaError_t e = cudaGraphInstantiate(exec, g, 0);
   cudaGraphDestroy(g);
@@ -706,7 +740,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   *out = nullptr;
   if (!valid_shape(theory, Nx, Ny, p) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
   if (p->integrator != SS_RK4 && p->integrator != SS_VERLET) return SS_ERR_ARG;
-  if (p->flags & ~(SS_FLAG_NO_GRAPH | SS_FLAG_NO_RESIDENT)) return SS_ERR_ARG;
+  if (p->flags & ~(SS_FLAG_NO_GRAPH | SS_FLAG_NO_RESIDENT | SS_FLAG_NO_SLABS)) return SS_ERR_ARG;
   if (theory == SS_THEORY_BABY_SKYRME && p->dmi_d) return SS_ERR_UNSUPPORTED;
   if (!std::isfinite(p->demag) || p->demag < 0.0 || p->demag_cycles < 0) return SS_ERR_ARG;
   if (p->demag != 0.0 && theory == SS_THEORY_CHIRAL_MAGNET && p->dtype != SS_F64)
@@ -805,6 +839,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (!cuda_ok(e, "cudaFuncSetAttribute")) { delete s; return SS_ERR_CUDA; }
     }
   }
+  int slots[3] = {1, 1, 1};
   for (int kind = 0; kind < 3 && s->ktheory != kBS; ++kind) {
     void* f = flow_func(s->ktheory, p->dtype, kind);
     const int smem = flow_smem(s->ktheory, p->dtype, kind);
@@ -817,10 +852,13 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     }
     s->cps[kind] = p->chunks_per_segment > 0 ? p->chunks_per_segment
                                              : choose_cps(L.nseg, Ny, s->batch, s->sms * o);
+    slots[kind] = s->sms * o;
   }
+  plan_slabs(s, p->chunks_per_segment, slots[KX] < slots[KY] ? slots[KX] : slots[KY]);
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
+    int join = 1;  // row_reduce waits for the last 2 * join nodes (slab schedule) or the last one
     if (s->demag != 0.0) {
       make_demag_step(s, cur, st, ev);
     } else if (s->ktheory == kBS) {
@@ -841,6 +879,53 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       }
       st.push_back(v);   // the whole step: phi', v', a', E, Q, KE
       ev.push_back(x0);  // a (-> acc(0), only used with cur == 0), E, Q
+    } else if (s->slabs > 1) {
+      // Row-slab pipelining (DESIGN 6.1): Y and X of one step as SLABS launches each over
+      // contiguous ranges of y-segments.  X_k reads rows that Y_{k-1}, Y_k, Y_{k+1} write (one
+      // chunk beyond its slab on either side) and overwrites a1, a2 rows that the same three
+      // read, so those are its only edges; the Y_k depend on the previous step's arrest flag
+      // alone.  X's CTAs fill the SMs that the tail of Y leaves idle.  Node order (also the
+      // order of the direct-launch path) is Y0 Y1 X0 Y2 X1 ... so that it is topological.
+      const int S = s->slabs;
+      const int NC = (s->Ny + FR - 1) / FR;
+      const int nsy = (NC + s->cps[KY] - 1) / s->cps[KY];
+      std::vector<int> lo(S + 1), iy(S);
+      for (int k = 0; k <= S; ++k) lo[k] = (int)((long long)nsy * k / S);
+      std::vector<std::pair<int, int>> order;  // (0 = Y, 1 = X; slab)
+      for (int k = 0; k < S; ++k) {
+        order.push_back({0, k});
+        if (k >= 1) order.push_back({1, k - 1});
+      }
+      order.push_back({1, S - 1});
+      for (int i = 0; i < (int)order.size(); ++i)
+        if (!order[i].first) iy[order[i].second] = i;
+      for (int i = 0; i < (int)order.size(); ++i) {
+        const int k = order[i].second, isx = order[i].first;
+        KernelNode n;
+        if (!make_flow_node(s, isx ? KX : KY, isx ? cur ^ 1 : cur, &n, lo[k], lo[k + 1] - lo[k])) {
+          ss_destroy(s);
+          return SS_ERR_CUDA;
+        }
+        if (!isx) {
+          n.back = {i + 1};  // the node before this step: the previous step's finalize
+        } else {
+          n.back = {i - iy[k]};
+          if (k >= 1) n.back.push_back(i - iy[k - 1]);
+          if (k + 1 < S) n.back.push_back(i - iy[k + 1]);
+        }
+        st.push_back(n);
+      }
+      KernelNode y, x, x0;  // the unsplit launches: ss_profile_step times these one by one
+      if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, KX, cur ^ 1, &x) ||
+          !make_flow_node(s, KX, cur, &x0)) {
+        ss_destroy(s);
+        return SS_ERR_CUDA;
+      }
+      s->prof_nodes[cur].push_back(y);
+      s->prof_nodes[cur].push_back(x);
+      make_reduce_nodes(s, 1, s->prof_nodes[cur]);
+      ev.push_back(x0);
+      join = S;
     } else {
       KernelNode y, x, x0;
       if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, KX, cur ^ 1, &x) ||
@@ -853,6 +938,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       ev.push_back(x0);
     }
     make_reduce_nodes(s, 1, st);
+    if (join > 1)
+      for (int k = 1; k <= 2 * join; ++k) st[st.size() - 2].back.push_back(k);
     make_reduce_nodes(s, 0, ev);
     if (!(s->flags & SS_FLAG_NO_GRAPH)) {
       int rc = build_graph(s, st, &s->step_exec[cur]);
@@ -1058,7 +1145,8 @@ int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_ker
   if (!s || !ms_host || !n_kernels || reps < 1) return SS_ERR_ARG;
   if (!s->fields_set) return SS_ERR_STATE;
   GUARD(s);
-  const int n = (int)s->step_nodes[0].size();
+  const bool split = !s->prof_nodes[0].empty();  // slab schedule: time the unsplit launches
+  const int n = (int)(split ? s->prof_nodes[0] : s->step_nodes[0]).size();
   *n_kernels = n;
   if (cap < n) return SS_ERR_ARG;
   std::vector<cudaEvent_t> ev(n + 1);
@@ -1066,7 +1154,7 @@ int ss_profile_step(ss_solver* s, int reps, double* ms_host, int cap, int* n_ker
   std::vector<double> acc(n, 0.0);
   int rc = SS_OK;
   for (int it = 0; it < reps && rc == SS_OK; ++it) {
-    auto& nodes = s->step_nodes[s->cur];
+    auto& nodes = split ? s->prof_nodes[s->cur] : s->step_nodes[s->cur];
     cudaError_t e = cudaEventRecord(ev[0], s->stream);
     for (int i = 0; i < n && e == cudaSuccess; ++i) {
       void* params[1] = {nodes[i].args.data()};
@@ -1149,12 +1237,14 @@ const char* ss_schedule_name(const ss_solver* s) {
   if (!s) return "";
   if (s->res_cl > 0) return "resident-cluster";
   if (s->ktheory == kBS) return "per-stage tile kernels";
+  if (s->slabs > 1) return "two-kernel, row slabs";
   return s->integrator == SS_VERLET ? "one-kernel verlet" : "two-kernel";
 }
 
 const char* ss_kernel_name(const ss_solver* s, int i) {
-  if (!s || i < 0 || i >= (int)s->step_nodes[0].size()) return "";
-  return s->step_nodes[0][i].name;
+  if (!s) return "";
+  const auto& nodes = s->prof_nodes[0].empty() ? s->step_nodes[0] : s->prof_nodes[0];
+  return i >= 0 && i < (int)nodes.size() ? nodes[i].name : "";
 }
 
 int64_t ss_launch_count(const ss_solver* s) { return s ? s->launches : 0; }

@@ -52,6 +52,7 @@ struct FlowArgs {
   const LatticeState* state;
   const double* Bb;               // [batch] Zeeman field per lattice
   int Nx, Ny, nseg, cps;          // cps = chunks per segment
+  int seg0;                       // first y-segment of this launch (row slabs, ss_api.cu)
   long long plane;                // Nx*Ny
   real hdt, dt, qdt2, hdt2;       // dt/2, dt, dt^2/4, dt^2/2
   real sdt2, sdt;                 // dt^2/6, dt/6
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   const int Nx = p.Nx, Ny = p.Ny;
   const int b = blockIdx.z, x0 = blockIdx.x * FW;
   const int NC = (Ny + FR - 1) / FR;
-  const int cs = blockIdx.y * p.cps, ce = min(cs + p.cps, NC);  // stencil chunks [cs, ce)
+  const int cs = (blockIdx.y + p.seg0) * p.cps, ce = min(cs + p.cps, NC);  // stencil chunks [cs, ce)
   const int f0 = max(cs - 1, 0), f1 = min(ce, NC - 1);          // fill chunks [f0, f1]
   const bool vz = KIND != KX ? (p.state[b].v_is_zero != 0) : false;
   const vreal Bz = vreal(real(p.Bb[b]));

@@ -28,6 +28,7 @@ RK4, VERLET = 0, 1
 OBS_ENERGY, OBS_CHARGE, OBS_ORDER = 0, 1, 2
 FLAG_NO_GRAPH = 1
 FLAG_NO_RESIDENT = 2
+FLAG_NO_SLABS = 4
 
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
            "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",

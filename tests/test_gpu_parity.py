@@ -397,7 +397,7 @@ def test_error_paths():
         assert e.value.code == ss.ERR_UNSUPPORTED
         assert ss.workspace_bytes(0, kw["Nx"], kw["Ny"], batch=kw.get("batch", 1)) == 0
     with pytest.raises(ss.SSError) as e:
-        ss.Solver(0, 64, 64, 0.2, flags=4)             # unknown flag bit
+        ss.Solver(0, 64, 64, 0.2, flags=8)             # unknown flag bit
     assert e.value.code == ss.ERR_ARG
     s = ss.Solver(0, 64, 64, 0.2, kappa=1.0, B=0.6)
     with pytest.raises(ss.SSError) as e:

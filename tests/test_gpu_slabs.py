@@ -1,0 +1,70 @@
+"""The row-slab schedule of the RK4 step (ss_api.cu `plan_slabs`: kernels Y and X split into four
+row slabs each that overlap inside the CUDA graph) against the unsplit two-kernel schedule and
+the oracle.  Only the launch geometry and the graph edges differ, so fields, E, Q, KE and the
+arrest log must be bitwise identical; a missing edge would show as a race on the rows at a slab
+seam.  The 4096^2 and 2048^2 full-size parity tests (tests/test_gpu_fullsize.py) run through this
+schedule by default; here it is forced on smaller lattices with one chunk per segment."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2603_24370_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _ss():
+    from paper_2603_24370_b200 import ss
+    return ss
+
+
+def _dev(a, dtype=torch.float64):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0", dtype=dtype).contiguous()
+
+
+def _cases():
+    # (workload, fp32?, uphill start so that steps arrest early, steps)
+    yield "cm", W.cm_quench(N=644), False, True, 12
+    yield "cm_f32", W.cm_quench(N=900), True, False, 12
+    yield "ah", W.ah_vortices(N=516, h=0.1, lam=2.0, count=2, min_sep=2.0), False, False, 8
+
+
+@pytest.mark.parametrize("case", ["cm", "cm_f32", "ah"])
+def test_slab_schedule_is_bitwise_identical_and_matches_the_oracle(case):
+    ss = _ss()
+    name, w, f32, uphill, steps = next(c for c in _cases() if c[0] == case)
+    td = torch.float32 if f32 else torch.float64
+    m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=w.B, K=w.K, lam=w.lam)
+    vel = (-0.06 * oracle.accel(m, w.fields[0]))[None] if uphill else None
+    outs = {}
+    for flags in (ss.FLAG_NO_SLABS, 0, ss.FLAG_NO_GRAPH):
+        s = ss.solver_for(w, dtype=ss.F32 if f32 else ss.F64, flags=flags, cps=1)
+        assert s.schedule() == ("two-kernel" if flags == ss.FLAG_NO_SLABS else "two-kernel, row slabs")
+        s.set_fields(_dev(w.fields, td), None if vel is None else _dev(vel, td))
+        s.step(steps)          # 8-step graph + single-step graphs
+        f, v = s.get_fields()
+        outs[flags] = (f.cpu(), v.cpu(), s.energy(), s.charge(), s.kinetic(), s.arrests(0))
+    ref = outs[ss.FLAG_NO_SLABS]
+    for flags in (0, ss.FLAG_NO_GRAPH):
+        o = outs[flags]
+        assert torch.equal(ref[0], o[0]) and torch.equal(ref[1], o[1]), flags
+        assert ref[2:] == o[2:], flags
+    if uphill:
+        assert ref[5][0][:1] == [1]
+    if not f32:
+        fl = oracle.Flow(m, w.dt)
+        fl.set_fields(w.fields[0], None if vel is None else vel[0])
+        fl.step(steps)
+        ophi, ovel = fl.get_fields()
+        assert np.abs(outs[0][0][0].numpy() - ophi).max() <= 1e-11
+        assert np.abs(outs[0][1][0].numpy() - ovel).max() <= 1e-10
+        assert outs[0][5][0] == fl.arrests()
+
+
+def test_slabs_are_not_used_where_they_do_not_pay():
+    ss = _ss()
+    assert ss.solver_for(W.cm_multi(N=1024)).schedule() == "two-kernel"          # < 3 waves
+    assert ss.solver_for(W.cm_sweep(batch=4, N=256)).schedule() == "two-kernel"   # batched
+    assert ss.solver_for(W.cm_quench(N=2048), integrator=ss.VERLET).schedule() == "one-kernel verlet"
+    assert ss.solver_for(W.cm_quench(N=4096)).schedule() == "two-kernel, row slabs"
