@@ -66,7 +66,8 @@ enum {
   SS_ERR_CUDA = -3,        /* CUDA runtime failure (text via ss_strerror)                   */
   SS_ERR_WORKSPACE = -4,   /* workspace NULL / too small / misaligned                       */
   SS_ERR_STATE = -5,       /* stepping or reading before ss_set_fields                      */
-  SS_ERR_NONFINITE = -6    /* an energy became NaN/Inf (values are still written)           */
+  SS_ERR_NONFINITE = -6,   /* an energy became NaN/Inf (values are still written)           */
+  SS_ERR_TOO_LARGE = -7    /* ss_render_noalloc: Nx * Ny exceeds SS_NOALLOC_MAX_SITES       */
 };
 
 /* Integrators.  SS_RK4 is the paper's example ("such as fourth-order Runge-Kutta").
@@ -200,6 +201,27 @@ enum { SS_OBS_ENERGY = 0,   /* site-form energy density e_i                     
        SS_OBS_CHARGE = 1,   /* CM: degree density; AH: flux density / 2 pi                     */
        SS_OBS_ORDER = 2 };  /* CM: n3; AH: |phi| (order-parameter magnitude)                   */
 int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double* minmax_host);
+
+/* Allocation-free variant of ss_render for callers that cannot allocate device memory (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): no handle
+ * -- ss_create instantiates CUDA graphs -- and no workspace.  The same kernels as ss_render on
+ * ONE lattice fields_dev (DEVICE, [C][Ny][Nx], dtype p->dtype), with their scratch (per-block
+ * extrema, non-finite flag) in a static device array inside the library: 256 KiB + 256 B that
+ * every GPU which loads the library holds until exit, sized for Nx * Ny <= SS_NOALLOC_MAX_SITES
+ * (larger lattices: SS_ERR_TOO_LARGE).  Read from p: dtype, kappa, B,
+ * K, lambda, dmi_d, mu, potential, potential_n, stream; everything else is ignored.  Outputs,
+ * all DEVICE memory of the caller: rgba_dev [Ny][Nx] RGBA8 (may be NULL: extrema only),
+ * minmax_dev double[2], nonfinite_dev int[1] (may be NULL; 1 when an interior value was NaN or
+ * Inf).  Asynchronous on p->stream: one 4-byte memset, two or three kernels, one 4-byte
+ * device-to-device copy; calls cudaMalloc, cudaFree or an allocating library routine never.
+ * The first call on a device looks up the array's address (cudaGetSymbolAddress, which may load
+ * the module): make one call per device before capturing.  All calls on a device share the
+ * array, which keeps the last call's contents (the call clears what must start at zero): calls
+ * that overlap on the GPU -- different streams, or graphs replayed concurrently -- race. */
+#define SS_NOALLOC_MAX_SITES (2048 * 2048)
+int ss_render_noalloc(int theory, int Nx, int Ny, double h, const ss_params* p, int observable,
+                      const void* fields_dev, void* rgba_dev, double* minmax_dev,
+                      int* nonfinite_dev);
 
 const char* ss_strerror(int code);
 

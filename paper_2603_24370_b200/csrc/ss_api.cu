@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1258,8 +1259,124 @@ const char* ss_strerror(int code) {
     case SS_ERR_WORKSPACE: return "workspace missing, too small or misaligned";
     case SS_ERR_STATE: return "fields not set";
     case SS_ERR_NONFINITE: return "non-finite energy";
+    case SS_ERR_TOO_LARGE: return "lattice exceeds SS_NOALLOC_MAX_SITES (2048 x 2048 sites) of ss_render_noalloc";
     default: return "unknown status";
   }
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Allocation-free entry point (include/ss.h ss_render_noalloc): the render kernels of
+// ss_render.cuh with their scratch -- the per-block extrema and the non-finite flag -- in a
+// file-scope device array instead of a caller workspace, so that no handle (ss_create builds
+// CUDA graphs, i.e. allocates) and no workspace is needed.  Every call on a device shares the
+// array; calls that overlap on the GPU race on it.
+namespace {
+
+constexpr long long NOALLOC_MAX_SITES = SS_NOALLOC_MAX_SITES;
+constexpr int NOALLOC_MAX_BLOCKS = (int)((NOALLOC_MAX_SITES + 255) / 256);
+constexpr int NOALLOC_FLAG_AT = 2 * NOALLOC_MAX_BLOCKS;  // the flag word sits after the partials
+constexpr int NOALLOC_MAX_DEVICES = 64;
+// [2 * NOALLOC_MAX_BLOCKS] block (min, max), then the non-finite flag: 256 KiB + 256 B per device
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_FLAG_AT + 32];
+
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol; the device address is
+// looked up once per device, with that device current, and cached here.
+double* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+std::mutex g_noalloc_mutex;
+
+int noalloc_scratch(int device, double** out) {
+  if (device < 0 || device >= NOALLOC_MAX_DEVICES) return SS_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[device]) {
+    double* ptr = nullptr;  // the caller has made `device` current
+    if (!cuda_ok(cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch), "cudaGetSymbolAddress") ||
+        !ptr)
+      return SS_ERR_CUDA;
+    g_noalloc_ptr[device] = ptr;
+  }
+  *out = g_noalloc_ptr[device];
+  return SS_OK;
+}
+
+template <int THEORY, typename real>
+int render_noalloc_t(const ss_solver* k, double* scratch, int obs, const void* fields_dev,
+                     void* rgba_dev, double* minmax_dev, int* nonfinite_dev) {
+  FlowArgs<real> fa;
+  memset(&fa, 0, sizeof(fa));
+  fill_constants(k, fa);
+  RenderArgs<real> r;
+  memset(&r, 0, sizeof(r));
+  const size_t sites = (size_t)k->Nx * k->Ny;
+  r.phi = (const real*)fields_dev;
+  r.nblocks = (int)((sites + 255) / 256);
+  r.part = scratch;
+  r.minmax = minmax_dev;
+  r.nonfinite = (int*)(scratch + NOALLOC_FLAG_AT);
+  r.rgba = (unsigned int*)rgba_dev;
+  r.Nx = k->Nx; r.Ny = k->Ny; r.obs = obs;
+  r.B = real(k->B);
+  // the array keeps the last call's contents: the flag must start at zero (the block partials
+  // [0, 2 nblocks) are all rewritten by observable_kernel before minmax_kernel reads them)
+  CK(cudaMemsetAsync(r.nonfinite, 0, sizeof(int), k->stream));
+  observable_kernel<THEORY, real><<<r.nblocks, 256, 0, k->stream>>>(fa, r);
+  minmax_kernel<real><<<1, 1024, 0, k->stream>>>(r);
+  if (rgba_dev) colormap_kernel<THEORY, real><<<r.nblocks, 256, 0, k->stream>>>(fa, r);
+  CK(cudaGetLastError());
+  if (nonfinite_dev)
+    CK(cudaMemcpyAsync(nonfinite_dev, r.nonfinite, sizeof(int), cudaMemcpyDeviceToDevice, k->stream));
+  return SS_OK;
+}
+
+}  // namespace
+
+extern "C" int ss_render_noalloc(int theory, int Nx, int Ny, double h, const ss_params* p,
+                                 int observable, const void* fields_dev, void* rgba_dev,
+                                 double* minmax_dev, int* nonfinite_dev) {
+  if (!p || !fields_dev || !minmax_dev || observable < 0 || observable > 2) return SS_ERR_ARG;
+  ss_params q = *p;
+  q.batch = 1;  // one lattice per call; workspace, B_batch, integrator and flags are not used
+  q.flags = 0;
+  if (!valid_shape(theory, Nx, Ny, &q) || !(h > 0.0) || !std::isfinite(h)) return SS_ERR_ARG;
+  if (theory == SS_THEORY_BABY_SKYRME && p->dmi_d) return SS_ERR_UNSUPPORTED;
+  if ((long long)Nx * Ny > NOALLOC_MAX_SITES) return SS_ERR_TOO_LARGE;
+  cudaPointerAttributes pa;
+  if (!cuda_ok(cudaPointerGetAttributes(&pa, fields_dev), "cudaPointerGetAttributes"))
+    return SS_ERR_CUDA;
+  if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return SS_ERR_ARG;
+  ss_solver k;  // host-side carrier of the constants only (never stepped, owns nothing)
+  k.theory = theory; k.dtype = p->dtype; k.Nx = Nx; k.Ny = Ny; k.batch = 1; k.h = h;
+  k.device = pa.device;
+  k.dt = 0.5 * h;
+  k.kappa = p->kappa; k.B = p->B; k.K = p->K; k.lambda = p->lambda;
+  k.mu = p->mu; k.pot = p->potential; k.potN = p->potential_n;
+  k.stream = (cudaStream_t)p->stream;
+  k.L.nseg = (Nx + SEG - 1) / SEG;
+  k.ktheory = theory == SS_THEORY_BABY_SKYRME ? kBS : theory;
+  for (int i = 0; i < 6; ++i) k.dmi[i] = 0.0;
+  if (theory == SS_THEORY_CHIRAL_MAGNET && p->dmi_d) {
+    k.ktheory = kCMG;
+    for (int i = 0; i < 6; ++i) {
+      if (!std::isfinite(p->dmi_d[i])) return SS_ERR_ARG;
+      k.dmi[i] = p->dmi_d[i];
+    }
+  }
+  GUARD(&k);
+  double* scratch = nullptr;
+  int rc = noalloc_scratch(k.device, &scratch);
+  if (rc != SS_OK) return rc;
+  const bool f64 = p->dtype == SS_F64;
+#define SS_NOALLOC_CASE(TH)                                                                        \
+  return f64 ? render_noalloc_t<TH, double>(&k, scratch, observable, fields_dev, rgba_dev,         \
+                                            minmax_dev, nonfinite_dev)                             \
+             : render_noalloc_t<TH, float>(&k, scratch, observable, fields_dev, rgba_dev,          \
+                                           minmax_dev, nonfinite_dev)
+  switch (k.ktheory) {
+    case kCM: SS_NOALLOC_CASE(kCM);
+    case kAH: SS_NOALLOC_CASE(kAH);
+    case kBS: SS_NOALLOC_CASE(kBS);
+    default:  SS_NOALLOC_CASE(kCMG);
+  }
+#undef SS_NOALLOC_CASE
+}

@@ -22,10 +22,11 @@ _lib = C.CDLL(LIB_PATH)
 THEORY_CHIRAL_MAGNET, THEORY_ABELIAN_HIGGS, THEORY_BABY_SKYRME = 0, 1, 2
 POT_STANDARD, POT_EASY_PLANE, POT_BROKEN = 0, 1, 2
 F64, F32 = 0, 1
-OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE = \
-    0, -1, -2, -3, -4, -5, -6
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_NONFINITE, ERR_TOO_LARGE = \
+    0, -1, -2, -3, -4, -5, -6, -7
 RK4, VERLET = 0, 1
 OBS_ENERGY, OBS_CHARGE, OBS_ORDER = 0, 1, 2
+NOALLOC_MAX_SITES = 2048 * 2048   # SS_NOALLOC_MAX_SITES of include/ss.h
 FLAG_NO_GRAPH = 1
 FLAG_NO_RESIDENT = 2
 FLAG_NO_SLABS = 4
@@ -33,7 +34,8 @@ FLAG_NO_SLABS = 4
 EXPORTS = ["ss_workspace_bytes", "ss_create", "ss_destroy", "ss_set_fields", "ss_get_fields",
            "ss_set_fields_host", "ss_get_fields_host", "ss_profile_step", "ss_kernel_name",
            "ss_step", "ss_energy", "ss_charge", "ss_kinetic", "ss_status", "ss_arrests",
-           "ss_launch_count", "ss_strerror", "ss_render", "ss_schedule_name"]
+           "ss_launch_count", "ss_strerror", "ss_render", "ss_schedule_name",
+           "ss_render_noalloc"]
 
 
 class ss_params(C.Structure):
@@ -73,6 +75,8 @@ _lib.ss_arrests.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int64), C.c_int64
 _lib.ss_launch_count.argtypes = [C.c_void_p]
 _lib.ss_render.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, _dp]
 _lib.ss_launch_count.restype = C.c_int64
+_lib.ss_render_noalloc.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(ss_params),
+                                   C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ss_strerror.argtypes = [C.c_int]
 _lib.ss_strerror.restype = C.c_char_p
 
@@ -278,6 +282,41 @@ class Solver:
 
     def launch_count(self) -> int:
         return _lib.ss_launch_count(self._h)
+
+
+def render_noalloc(theory, h, fields, minmax, *, rgba=None, nonfinite=None, observable=OBS_ENERGY,
+                   dtype=F64, kappa=0.0, B=0.0, K=0.0, lam=0.0, dmi=None, mu=0.0, pot=POT_STANDARD,
+                   potN=3, stream=None) -> None:
+    """ss_render_noalloc: extrema (and image) of one observable of ONE lattice `fields`
+    ([C][Ny][Nx] CUDA tensor) with no handle, no workspace and no device allocation: the caller
+    passes every output -- minmax (2 float64), rgba ([Ny][Nx][4] uint8, optional), nonfinite
+    (1 int32, optional), all CUDA tensors on the device of `fields`.  Asynchronous on `stream`
+    (default: torch's current stream).  Lattices of more than NOALLOC_MAX_SITES sites are
+    rejected; calls that overlap on the GPU race on the library's static scratch."""
+    C_, Ny, Nx = (int(x) for x in fields.shape)
+    want = torch.float64 if dtype == F64 else torch.float32
+    if not (fields.is_cuda and fields.is_contiguous() and fields.dtype == want and
+            C_ == (4 if theory == THEORY_ABELIAN_HIGGS else 3)):
+        raise ValueError("fields: need a contiguous [C][Ny][Nx] CUDA tensor of the solver dtype")
+    if not (minmax.is_cuda and minmax.dtype == torch.float64 and minmax.numel() == 2 and
+            minmax.is_contiguous() and minmax.device == fields.device):
+        raise ValueError("minmax: need 2 contiguous float64 on the device of fields")
+    if rgba is not None and not (rgba.is_cuda and rgba.dtype == torch.uint8 and rgba.is_contiguous()
+                                 and tuple(rgba.shape) == (Ny, Nx, 4) and rgba.device == fields.device):
+        raise ValueError("rgba: need a contiguous [Ny][Nx][4] uint8 CUDA tensor")
+    if nonfinite is not None and not (nonfinite.is_cuda and nonfinite.dtype == torch.int32 and
+                                      nonfinite.numel() == 1 and nonfinite.device == fields.device):
+        raise ValueError("nonfinite: need 1 int32 on the device of fields")
+    p, keep = _params(dtype, 1, 0.0, kappa, B, K, lam, None, 0, 0, dmi=dmi, mu=mu, pot=pot, potN=potN)
+    st = stream if stream is not None else torch.cuda.current_stream(fields.device)
+    p.stream = st.cuda_stream
+    _check(_lib.ss_render_noalloc(int(theory), Nx, Ny, float(h), C.byref(p), int(observable),
+                                  C.c_void_p(fields.data_ptr()),
+                                  C.c_void_p(rgba.data_ptr()) if rgba is not None else None,
+                                  C.c_void_p(minmax.data_ptr()),
+                                  C.c_void_p(nonfinite.data_ptr()) if nonfinite is not None else None),
+           "ss_render_noalloc")
+    del keep
 
 
 def solver_for(w, *, dtype=F64, flags=0, device="cuda:0", log_cap=0, cps=0,
