@@ -581,7 +581,11 @@ void plan_slabs(ss_solver* s, int user_cps, int slots) {
   s->cps[KX] = s->cps[KY] = cps;
 }
 
-void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>& out) {
+// row_reduce of rows [row0, row1) alone (the slab schedule finishes the rows of a slab as soon as
+// its X is done)
+KernelNode make_row_reduce_node(const ss_solver* s, int row0, int row1);
+void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>& out,
+                       bool finalize_only = false) {
   ReduceArgs a;
   memset(&a, 0, sizeof(a));
   a.part_e = s->part(0);
@@ -593,6 +597,7 @@ void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>&
   a.log_cap = s->log_cap;
   a.Ny = s->Ny; a.nseg = s->L.nseg; a.advance = advance;
   a.h2 = s->h * s->h;
+  a.row0 = 0; a.row1 = s->Ny;
   KernelNode r;
   r.func = (void*)row_reduce_kernel;
   r.grid = dim3((s->Ny + 7) / 8, s->batch, 1);
@@ -600,13 +605,25 @@ void make_reduce_nodes(const ss_solver* s, int advance, std::vector<KernelNode>&
   r.smem = 0;
   set_args(r, &a, sizeof(a));
   r.name = "row_reduce";
-  out.push_back(r);
+  if (!finalize_only) out.push_back(r);
   KernelNode f = r;
   f.name = "finalize_arrest";
   f.func = (void*)finalize_kernel;
   f.grid = dim3(s->batch, 1, 1);
   f.block = dim3(1024, 1, 1);
   out.push_back(f);
+}
+
+KernelNode make_row_reduce_node(const ss_solver* s, int row0, int row1) {
+  std::vector<KernelNode> both;
+  make_reduce_nodes(s, 1, both);
+  KernelNode r = both[0];
+  ReduceArgs a;
+  memcpy(&a, r.args.data(), sizeof(a));
+  a.row0 = row0; a.row1 = row1;
+  set_args(r, &a, sizeof(a));
+  r.grid = dim3((row1 - row0 + 7) / 8, s->batch, 1);
+  return r;
 }
 
 int launch_nodes(ss_solver* s, std::vector<KernelNode>& nodes) {
@@ -859,7 +876,7 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
-    int join = 1;  // row_reduce waits for the last 2 * join nodes (slab schedule) or the last one
+    int join = 1;  // > 1: slab schedule with that many slabs
     if (s->demag != 0.0) {
       make_demag_step(s, cur, st, ev);
     } else if (s->ktheory == kBS) {
@@ -885,29 +902,42 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       // contiguous ranges of y-segments.  X_k reads rows that Y_{k-1}, Y_k, Y_{k+1} write (one
       // chunk beyond its slab on either side) and overwrites a1, a2 rows that the same three
       // read, so those are its only edges; the Y_k depend on the previous step's arrest flag
-      // alone.  X's CTAs fill the SMs that the tail of Y leaves idle.  Node order (also the
-      // order of the direct-launch path) is Y0 Y1 X0 Y2 X1 ... so that it is topological.
+      // alone.  X's CTAs fill the SMs that the tail of Y leaves idle, and the rows of a slab are
+      // reduced (R_k) as soon as X_k is done, so that only the last slab's row_reduce and the
+      // finalize are serial (0.7931 vs 0.7949 ms with one row_reduce at the end).  Node order (also
+      // the order of the direct-launch path) is Y0 Y1 X0 R0 Y2 X1 R1 ...: topological.
       const int S = s->slabs;
       const int NC = (s->Ny + FR - 1) / FR;
       const int nsy = (NC + s->cps[KY] - 1) / s->cps[KY];
-      std::vector<int> lo(S + 1), iy(S);
+      std::vector<int> lo(S + 1), iy(S), ix(S);
       for (int k = 0; k <= S; ++k) lo[k] = (int)((long long)nsy * k / S);
-      std::vector<std::pair<int, int>> order;  // (0 = Y, 1 = X; slab)
+      std::vector<std::pair<int, int>> order;  // (0 = Y, 1 = X, 2 = row_reduce; slab)
       for (int k = 0; k < S; ++k) {
         order.push_back({0, k});
-        if (k >= 1) order.push_back({1, k - 1});
+        if (k >= 1) { order.push_back({1, k - 1}); order.push_back({2, k - 1}); }
       }
       order.push_back({1, S - 1});
-      for (int i = 0; i < (int)order.size(); ++i)
-        if (!order[i].first) iy[order[i].second] = i;
+      order.push_back({2, S - 1});
       for (int i = 0; i < (int)order.size(); ++i) {
-        const int k = order[i].second, isx = order[i].first;
+        if (order[i].first == 0) iy[order[i].second] = i;
+        if (order[i].first == 1) ix[order[i].second] = i;
+      }
+      const int rows_per_seg = s->cps[KY] * FR;
+      for (int i = 0; i < (int)order.size(); ++i) {
+        const int k = order[i].second, kind = order[i].first;
         KernelNode n;
-        if (!make_flow_node(s, isx ? KX : KY, isx ? cur ^ 1 : cur, &n, lo[k], lo[k + 1] - lo[k])) {
+        if (kind == 2) {
+          const int r1 = lo[k + 1] * rows_per_seg;
+          n = make_row_reduce_node(s, lo[k] * rows_per_seg, r1 < s->Ny ? r1 : s->Ny);
+          n.back = {i - ix[k]};  // X_k (which waited for Y_k: the KE partials of these rows)
+          st.push_back(n);
+          continue;
+        }
+        if (!make_flow_node(s, kind ? KX : KY, kind ? cur ^ 1 : cur, &n, lo[k], lo[k + 1] - lo[k])) {
           ss_destroy(s);
           return SS_ERR_CUDA;
         }
-        if (!isx) {
+        if (kind == 0) {
           n.back = {i + 1};  // the node before this step: the previous step's finalize
         } else {
           n.back = {i - iy[k]};
@@ -938,9 +968,9 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       st.push_back(x);  // a1, a2, E, Q on the new state
       ev.push_back(x0);
     }
-    make_reduce_nodes(s, 1, st);
-    if (join > 1)
-      for (int k = 1; k <= 2 * join; ++k) st[st.size() - 2].back.push_back(k);
+    make_reduce_nodes(s, 1, st, join > 1);
+    if (join > 1)  // finalize waits for the row_reduce of every slab (3 nodes per slab)
+      for (int k = 1; k <= 3 * join; ++k) st.back().back.push_back(k);
     make_reduce_nodes(s, 0, ev);
     if (!(s->flags & SS_FLAG_NO_GRAPH)) {
       int rc = build_graph(s, st, &s->step_exec[cur]);

@@ -31,6 +31,7 @@ struct ReduceArgs {
   long long log_cap;
   int Ny, nseg, advance;
   double h2;             // h*h
+  int row0, row1;        // row_reduce: this launch finishes rows [row0, row1)
 };
 
 // Aligned pairwise tree over the 32 lanes of a warp (lane l holds element l):

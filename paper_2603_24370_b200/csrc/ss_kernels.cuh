@@ -33,9 +33,9 @@ __device__ __forceinline__ double chunk_tree(const double* src, long long first,
 // One warp per lattice row: finishes the x-tree over the nseg segment partials of that row.
 __global__ void __launch_bounds__(256) row_reduce_kernel(const __grid_constant__ ReduceArgs p) {
   const int b = blockIdx.y;
-  const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int row = p.row0 + blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
-  if (row >= p.Ny) return;
+  if (row >= p.row1) return;
   int P = 32;
   while (P < p.nseg) P <<= 1;
   const int m = P / 32;
