@@ -60,6 +60,8 @@ def parse_args():
     ap.add_argument("--integrator", default="rk4", choices=["rk4", "verlet"],
                     help="rk4 = the metric's flow step (default); verlet = SURVEY 8(f) NEXT-1")
     ap.add_argument("--cps", type=int, default=0, help="chunks per segment (0 = auto)")
+    ap.add_argument("--no-slabs", action="store_true",
+                    help="SS_FLAG_NO_SLABS: whole-lattice launches of kernels Y and X (ncu captures)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0,
                     help="target CPU time of the oracle sample")
     ap.add_argument("--sustained-seconds", type=float, default=2.5,
@@ -359,6 +361,7 @@ def run_ours(args):
     R = 8 if dtname == "f64" else 4
     host = torch.from_numpy(w.fields).to(tdt).contiguous().pin_memory()
     s = ss.solver_for(w, dtype=dtype, device=str(dev), cps=args.cps,
+                      flags=ss.FLAG_NO_SLABS if args.no_slabs else 0,
                       integrator=ss.VERLET if args.integrator == "verlet" else ss.RK4)
     s.set_fields(host.to(dev))
     sites = w.interior_sites
@@ -448,6 +451,11 @@ def run_ours(args):
                 "shared memory: nothing streams from HBM, no HBM roofline applies); the kernels "
                 "listed here are the general two-kernel schedule of the same solver, launched one "
                 "by one by ss_profile_step, for comparison")
+    if s.schedule() == "two-kernel, row slabs":
+        note = ("ss_step replays kernels Y and X as 4 row-slab launches each that overlap inside the "
+                "graph (ms_graph < ms_sum_of_kernels); the per-kernel times here are whole-lattice "
+                "launches of the same kernels, one by one (ss_profile_step), which is also what "
+                "the ncu capture behind `traffic` holds (bench.py --no-slabs)")
     roofline = {
         "note": note,
         "bound": "hbm", "limiter": kern[dom]["limiter"],
