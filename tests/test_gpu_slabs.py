@@ -68,3 +68,23 @@ def test_slabs_are_not_used_where_they_do_not_pay():
     assert ss.solver_for(W.cm_sweep(batch=4, N=256)).schedule() == "two-kernel"   # batched
     assert ss.solver_for(W.cm_quench(N=2048), integrator=ss.VERLET).schedule() == "one-kernel verlet"
     assert ss.solver_for(W.cm_quench(N=4096)).schedule() == "two-kernel, row slabs"
+
+
+def test_slab_schedule_at_bench_size_is_bitwise_identical():
+    # 4096^2 fp64 (the metric's workload) and 2048^2 Abelian Higgs with the default segment length:
+    # 19 steps = two 8-step graphs + three single-step graphs, against whole-lattice launches
+    ss = _ss()
+    for w in (W.baseline_config(4), W.baseline_config(3)):
+        outs = []
+        for flags in (ss.FLAG_NO_SLABS, 0):
+            s = ss.solver_for(w, flags=flags)
+            s.set_fields(_dev(w.fields))
+            s.step(19)
+            f, v = s.get_fields()
+            outs.append((f, v, s.energy(), s.charge(), s.kinetic(), s.arrests(0), s.schedule()))
+            del s
+        assert outs[0][6] == "two-kernel" and outs[1][6] == "two-kernel, row slabs"
+        assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+        assert outs[0][2:6] == outs[1][2:6]
+        del outs
+        torch.cuda.empty_cache()
