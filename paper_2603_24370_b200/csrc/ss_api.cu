@@ -883,9 +883,13 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       if (s->integrator == SS_VERLET) {
         st.push_back(make_bs_node(s, 5, cur));  // the whole step: phi', v', a', E, Q, KE
       } else {
+        // stage 2 (phi, v -> a2) and stage 3 (phi, v, a1 -> a3) do not depend on one another:
+        // both wait for the previous step's finalize only and share the device
         st.push_back(make_bs_node(s, 2, cur));
         st.push_back(make_bs_node(s, 3, cur));
+        st.back().back = {2};
         st.push_back(make_bs_node(s, 4, cur));
+        st.back().back = {1, 2};
         st.push_back(make_bs_node(s, 1, cur ^ 1));  // a1, E, Q on the new field
       }
       ev.push_back(make_bs_node(s, 1, cur));
