@@ -88,3 +88,26 @@ def test_slab_schedule_at_bench_size_is_bitwise_identical():
         assert outs[0][2:6] == outs[1][2:6]
         del outs
         torch.cuda.empty_cache()
+
+
+def test_profile_step_under_the_slab_schedule_advances_like_step():
+    # ss_profile_step times whole-lattice launches of the same kernels (one by one); the state it
+    # leaves must be the one ss_step leaves
+    ss = _ss()
+    w = W.cm_quench(N=644)
+    a = ss.solver_for(w, cps=1)
+    b = ss.solver_for(w, cps=1)
+    assert a.schedule() == "two-kernel, row slabs"
+    for s in (a, b):
+        s.set_fields(_dev(w.fields))
+        s.step(2)
+    prof = a.profile_step(3)
+    b.step(3)
+    assert [n for n, _ in prof] == ["flow_y_stage34_combine_project_ke", "flow_x_grad_energy_charge_stage2",
+                                    "row_reduce", "finalize_arrest"]
+    a.step(4)
+    b.step(4)
+    fa, va = a.get_fields()
+    fb, vb = b.get_fields()
+    assert torch.equal(fa, fb) and torch.equal(va, vb)
+    assert a.energy() == b.energy() and a.status()["steps"] == b.status()["steps"] == 9
