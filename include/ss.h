@@ -202,8 +202,10 @@ enum { SS_OBS_ENERGY = 0,   /* site-form energy density e_i                     
        SS_OBS_ORDER = 2 };  /* CM: n3; AH: |phi| (order-parameter magnitude)                   */
 int ss_render(ss_solver* s, int observable, int lattice, void* rgba_dev, double* minmax_host);
 
-/* Allocation-free variant of ss_render for callers that cannot allocate device memory (code
- * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): no handle
+/* Allocation-free variant of ss_render (the same operation: device-side
+ * extrema and the colour-mapped image of an observable; DESIGN R17) for callers that cannot
+ * allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): no handle
  * -- ss_create instantiates CUDA graphs -- and no workspace.  The same kernels as ss_render on
  * ONE lattice fields_dev (DEVICE, [C][Ny][Nx], dtype p->dtype), with their scratch (per-block
  * extrema, non-finite flag) in a static device array inside the library: 256 KiB + 256 B that
