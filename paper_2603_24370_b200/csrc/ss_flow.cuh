@@ -26,6 +26,9 @@
 //      results with coalesced row stores and contributes to the row-segment partial sums of the
 //      canonical tree (warp xor-shuffle tree, then low half + high half after the next barrier).
 // No y-halo is ever re-read from HBM except one warm-up chunk per segment end.
+// A launch covers the y-segments [seg0, seg0 + gridDim.y): all of them, or -- on large single
+// lattices -- one row slab of the step's graph, in which X of a slab starts as soon as Y of the
+// slab and of its two neighbours is done (ss_api.cu plan_slabs).
 #pragma once
 #include <cuda.h>
 
