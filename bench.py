@@ -268,9 +268,10 @@ KERNEL_UNITS = {
 }
 STEP_UNITS_SURVEY = 21                          # stage fields materialised
 
-# kernel name in bench.py -> the KIND template argument of flow_kernel<THEORY, real, KIND>
-KERNEL_KIND = {"flow_x_grad_energy_charge_stage2": 0, "flow_y_stage34_combine_project_ke": 1,
-               "flow_v_verlet_step_energy_charge_ke": 2}
+# kernel name in bench.py -> the KIND template argument(s) of flow_kernel<THEORY, real, KIND>
+# (kernel X is KX = 0 inside the row-slab schedule and KXD = 3 elsewhere in fp64, ss_flow.cuh)
+KERNEL_KIND = {"flow_x_grad_energy_charge_stage2": (0, 3), "flow_y_stage34_combine_project_ke": (1,),
+               "flow_v_verlet_step_energy_charge_ke": (2,)}
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 
 
@@ -291,7 +292,7 @@ def ncu_traffic(workload_key, integrator, kernel):
             col = None
             for i, nm in enumerate(names):
                 m = re.search(r"flow_kernel<\s*\d+\s*,\s*\w+\s*,\s*(\d+)\s*>", nm)
-                if m and kind is not None and int(m.group(1)) == kind:
+                if m and kind is not None and int(m.group(1)) in kind:
                     col = i
             if col is None:
                 continue

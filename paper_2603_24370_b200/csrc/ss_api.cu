@@ -159,7 +159,8 @@ struct ss_solver {
   int flags;
   bool fields_set;
   int cur;  // which ping-pong buffer holds (phi, v)
-  int cps[3];  // chunks per y-segment of flow kernels X, Y, V
+  int cps[4];  // chunks per y-segment of flow kernels X, Y, V, XD
+  int xkind;   // KX, or KXD (phi by TMA straight into ring A: fp64, not Abelian Higgs, no row slabs)
   int integrator;
   int ktheory;    // kernel family: kCM, kAH or kCMG (chiral magnet with a DMI table)
   double dmi[6];  // (d_x, d_y) of the table
@@ -221,12 +222,13 @@ EncodeTiledFn encode_tiled() {
 
 // field array [batch*C][Ny][Nx] as a 3-D tensor; box = {FW + 2*XPAD, FR, C} starting 16 bytes
 // left of the strip (XPAD = 2 doubles / 4 floats); zero fill outside
-bool make_tmap(const ss_solver* s, void* base, CUtensorMap* out) {
+bool make_tmap(const ss_solver* s, void* base, CUtensorMap* out, bool per_component = false) {
   EncodeTiledFn enc = encode_tiled();
   if (!enc) { snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled unavailable"); return false; }
   cuuint64_t dims[3] = {(cuuint64_t)s->Nx, (cuuint64_t)s->Ny, (cuuint64_t)s->batch * s->C};
   cuuint64_t strides[2] = {(cuuint64_t)s->Nx * s->R, (cuuint64_t)s->Nx * s->Ny * s->R};
-  cuuint32_t box[3] = {(cuuint32_t)(FW + 32 / s->R), (cuuint32_t)FR, (cuuint32_t)s->C};
+  cuuint32_t box[3] = {(cuuint32_t)(FW + 32 / s->R), (cuuint32_t)FR,
+                       (cuuint32_t)(per_component ? 1 : s->C)};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = enc(out, s->dtype == SS_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
                                            : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
@@ -242,6 +244,8 @@ bool make_tmap(const ss_solver* s, void* base, CUtensorMap* out) {
 
 template <int THEORY, typename real>
 void* flow_func_t(int kind) {
+  if constexpr (sizeof(real) == 8 && THEORY != kAH)
+    if (kind == KXD) return (void*)flow_kernel<THEORY, real, KXD>;
   return kind == KX   ? (void*)flow_kernel<THEORY, real, KX>
          : kind == KY ? (void*)flow_kernel<THEORY, real, KY>
                       : (void*)flow_kernel<THEORY, real, KV>;
@@ -255,6 +259,8 @@ void* flow_func(int theory, int dtype, int kind) {
 }
 template <int THEORY, typename real>
 int flow_smem_t(int kind) {
+  if constexpr (sizeof(real) == 8 && THEORY != kAH)
+    if (kind == KXD) return FlowCfg<THEORY, real, KXD>::SMEM;
   return kind == KX   ? FlowCfg<THEORY, real, KX>::SMEM
          : kind == KY ? FlowCfg<THEORY, real, KY>::SMEM
                       : FlowCfg<THEORY, real, KV>::SMEM;
@@ -269,6 +275,8 @@ int flow_smem(int theory, int dtype, int kind) {
 
 template <int THEORY, typename real>
 int flow_threads_t(int kind) {
+  if constexpr (sizeof(real) == 8 && THEORY != kAH)
+    if (kind == KXD) return FlowCfg<THEORY, real, KXD>::THREADS;
   return kind == KX   ? FlowCfg<THEORY, real, KX>::THREADS
          : kind == KY ? FlowCfg<THEORY, real, KY>::THREADS
                       : FlowCfg<THEORY, real, KV>::THREADS;
@@ -313,7 +321,8 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out, int s
   if (!make_tmap(s, s->phi(in), &a.tm[0]) || !make_tmap(s, s->vel(in), &a.tm[1]) ||
       !make_tmap(s, s->acc(kind == KV ? in : 0), &a.tm[2]) || !make_tmap(s, s->acc(1), &a.tm[3]))
     return false;
-  if (kind == KX) {
+  if (kind == KXD && !make_tmap(s, s->phi(in), &a.tm[2], true)) return false;  // phi, one component per box
+  if (kind == KX || kind == KXD) {
     a.out0 = (real*)s->acc(0); a.out1 = (real*)s->acc(1);
     a.part0 = s->part(0); a.part1 = s->part(1);
   } else if (kind == KV) {
@@ -335,7 +344,7 @@ bool make_flow_node(const ss_solver* s, int kind, int in, KernelNode* out, int s
   n.block = dim3(flow_threads(s->ktheory, s->dtype, kind), 1, 1);
   n.smem = (size_t)flow_smem(s->ktheory, s->dtype, kind);
   set_args(n, &a, sizeof(a));
-  n.name = kind == KX   ? "flow_x_grad_energy_charge_stage2"
+  n.name = (kind == KX || kind == KXD) ? "flow_x_grad_energy_charge_stage2"
            : kind == KY ? "flow_y_stage34_combine_project_ke"
                         : "flow_v_verlet_step_energy_charge_ke";
   *out = n;
@@ -858,7 +867,9 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     }
   }
   int slots[3] = {1, 1, 1};
-  for (int kind = 0; kind < 3 && s->ktheory != kBS; ++kind) {
+  const bool has_xd = p->dtype == SS_F64 && s->ktheory != kAH && s->ktheory != kBS;
+  s->cps[KXD] = 1;
+  for (int kind = 0; kind < (has_xd ? 4 : 3) && s->ktheory != kBS; ++kind) {
     void* f = flow_func(s->ktheory, p->dtype, kind);
     const int smem = flow_smem(s->ktheory, p->dtype, kind);
     e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -870,9 +881,13 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
     }
     s->cps[kind] = p->chunks_per_segment > 0 ? p->chunks_per_segment
                                              : choose_cps(L.nseg, Ny, s->batch, s->sms * o);
-    slots[kind] = s->sms * o;
+    if (kind < 3) slots[kind] = s->sms * o;
   }
   plan_slabs(s, p->chunks_per_segment, slots[KX] < slots[KY] ? slots[KX] : slots[KY]);
+  // Without row slabs kernel X takes phi by TMA straight into its ring (ss_flow.cuh KXD: 4 CTAs
+  // per SM; 256 x 256^2 0.924 vs 0.940 ms, cm 1024^2 0.075 vs 0.078).  Inside the slab schedule
+  // its single TMA stage waits longer while Y streams (cm 4096^2 0.807 vs 0.793): KX there.
+  s->xkind = (has_xd && s->slabs == 0 && s->integrator == SS_RK4) ? KXD : KX;
   for (int cur = 0; cur < 2; ++cur) {
     auto& st = s->step_nodes[cur];
     auto& ev = s->eval_nodes[cur];
@@ -963,8 +978,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
       join = S;
     } else {
       KernelNode y, x, x0;
-      if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, KX, cur ^ 1, &x) ||
-          !make_flow_node(s, KX, cur, &x0)) {
+      if (!make_flow_node(s, KY, cur, &y) || !make_flow_node(s, s->xkind, cur ^ 1, &x) ||
+          !make_flow_node(s, s->xkind, cur, &x0)) {
         ss_destroy(s);
         return SS_ERR_CUDA;
       }

@@ -41,7 +41,7 @@ namespace ss {
 constexpr int FW = SEG;             // strip width = row segment of the reduction tree
 constexpr int FR = 4;               // rows per chunk
 constexpr int FWP = FW + 2 * HALO;  // ring width
-constexpr int KX = 0, KY = 1, KV = 2;
+constexpr int KX = 0, KY = 1, KV = 2, KXD = 3;  // KXD: kernel X with phi delivered into ring A (fp64)
 
 template <typename real>
 struct FlowArgs {
@@ -119,24 +119,37 @@ struct FlowCfg {
   static constexpr int LX = FW / VEC;                            // threads per row
   static constexpr int THREADS = LX * ROWT;
   static constexpr int RING = RING_ROWS;
-  static constexpr int NST = KIND == KY ? 1 : 2;                 // TMA stages
+  // KXD (fp64 chiral magnet, schedules without row slabs): kernel X's ring A is phi itself, so TMA
+  // delivers phi straight into a 16-row ring A (four chunk slots, one {68, 4, 1} box per
+  // component) and only v passes through a single stage buffer; the CTA shrinks from 72 to 55 KB
+  // and 116 registers: 4 CTAs per SM.  Same arithmetic, bitwise the same results as KX.
+  static constexpr bool ISX = KIND == KX || KIND == KXD;
+  static constexpr bool DIRECT = KIND == KXD;
+  static constexpr int RINGA = DIRECT ? 16 : RING;               // rows of ring A
+  static constexpr int NST = (KIND == KY || DIRECT) ? 1 : 2;     // TMA stages
   static constexpr int XPAD = 16 / (int)sizeof(real);            // box starts 16-byte aligned
   static constexpr int RAWW = FW + 2 * XPAD;                     // staged width (>= FWP)
   static constexpr int BOXB = C * FR * RAWW * (int)sizeof(real); // bytes one TMA box delivers
   static constexpr int ARRB = (BOXB + 127) / 128 * 128;          // 128-byte aligned slot
-  static constexpr int NARR = KIND == KX ? 2 : (KIND == KY ? 4 : 3);  // phi, v (, a1 (, a2))
+  static constexpr int NARR = ISX ? 2 : (KIND == KY ? 4 : 3);  // phi, v (, a1 (, a2))
   static constexpr int NRING = KIND == KV ? 1 : 2;
-  static constexpr int STAGEB = NARR * ARRB;
+  static constexpr int STAGEB = (DIRECT ? 1 : NARR) * ARRB;      // DIRECT: v only
   static constexpr int OFF_RING = NST * STAGEB;
-  static constexpr int RP = RING * FWP;                          // elements of one ring plane
-  static constexpr int RINGN = C * RP;                           // elements of one ring
-  static constexpr int OFF_RED = OFF_RING + NRING * RINGN * (int)sizeof(real);
+  static constexpr int RP = RING * FWP;                          // elements of one plane of ring B
+  static constexpr int RPA = RINGA * FWP;                        // ... of ring A
+  static constexpr int RINGN = C * RP;                           // elements of ring B
+  static constexpr int OFF_RED = OFF_RING + (C * RPA + (NRING - 1) * RINGN) * (int)sizeof(real);
   static constexpr int OFF_BAR = OFF_RED + 2 * 3 * FR * 2 * (int)sizeof(double);
   static constexpr int SMEM = OFF_BAR + NST * 8;
   static constexpr int FITB = (227 * 1024) / (SMEM + 1024);      // CTAs per SM that fit
-  static constexpr int WANTB = VEC == 2 ? MINB_F32V : MINB_F64;
+  static constexpr int WANTB = VEC == 2 ? MINB_F32V : (DIRECT ? MINB_F64 + 1 : MINB_F64);
+  static_assert(!DIRECT || sizeof(real) == 8, "KXD is an fp64 kernel");
   static constexpr int MINB = FITB < 1 ? 1 : (FITB < WANTB ? FITB : WANTB);
   static_assert(FR % SPT == 0 && RING >= 3 * FR + 2, "ring too small");
+  static_assert(!DIRECT || (RAWW == FWP && RINGA == 4 * FR && ARRB == BOXB), "DIRECT layout");
+  __device__ __forceinline__ static int ring_row_a(int gy) {
+    return DIRECT ? (gy & (RINGA - 1)) : ring_row(gy);
+  }
   __device__ __forceinline__ static int ring_row(int gy) {       // gy >= -RING
     return (RING & (RING - 1)) == 0 ? (gy & (RING - 1)) : (int)((unsigned)(gy + RING) % RING);
   }
@@ -183,13 +196,13 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
                                   FlowCfg<THEORY, real, KIND>::MINB)
     flow_kernel(const __grid_constant__ FlowArgs<real> p) {
   using Cfg = FlowCfg<THEORY, real, KIND>;
-  constexpr int C = Cfg::C, RP = Cfg::RP, SPT = Cfg::SPT, NST = Cfg::NST, VEC = Cfg::VEC;
+  constexpr int C = Cfg::C, RP = Cfg::RP, RPA = Cfg::RPA, SPT = Cfg::SPT, NST = Cfg::NST, VEC = Cfg::VEC;
   using vreal = typename VecOf<real, VEC>::type;
   using Th = typename TheoryOf<THEORY, vreal>::type;
-  constexpr int NQ = KIND == KX ? 2 : (KIND == KY ? 1 : 3);  // partial-sum quantities
+  constexpr int NQ = Cfg::ISX ? 2 : (KIND == KY ? 1 : 3);  // partial-sum quantities
   extern __shared__ __align__(128) unsigned char smem[];
   real* ringA = reinterpret_cast<real*>(smem + Cfg::OFF_RING);  // X: phi    Y: phi3   V: phi'
-  real* ringB = ringA + (Cfg::NRING - 1) * Cfg::RINGN;          // X: phi2   Y: phi4
+  real* ringB = ringA + (Cfg::NRING - 1) * C * RPA;             // X: phi2   Y: phi4
   double* red = reinterpret_cast<double*>(smem + Cfg::OFF_RED); // [2 parity][3 q][FR][2 halves]
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + Cfg::OFF_BAR);
 
@@ -200,7 +213,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   const int NC = (Ny + FR - 1) / FR;
   const int cs = (blockIdx.y + p.seg0) * p.cps, ce = min(cs + p.cps, NC);  // stencil chunks [cs, ce)
   const int f0 = max(cs - 1, 0), f1 = min(ce, NC - 1);          // fill chunks [f0, f1]
-  const bool vz = KIND != KX ? (p.state[b].v_is_zero != 0) : false;
+  const bool vz = !Cfg::ISX ? (p.state[b].v_is_zero != 0) : false;
   const vreal Bz = vreal(real(p.Bb[b]));
 
   if (tid == 0) {
@@ -214,11 +227,19 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
   auto issue = [&](int f) {
     unsigned char* st = smem + ((f - f0) % NST) * Cfg::STAGEB;
     uint64_t* bar = &full[(f - f0) % NST];
-    const int narr = KIND == KX ? 2 : (KIND == KY ? (vz ? 2 : 4) : (vz ? 2 : 3));
+    const int narr = Cfg::ISX ? 2 : (KIND == KY ? (vz ? 2 : 4) : (vz ? 2 : 3));
     mbar_expect_tx(bar, (uint32_t)(narr * Cfg::BOXB));
+    if constexpr (Cfg::DIRECT) {  // phi: one {68, 4, 1} box per component into the chunk's ring slot
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+        tma_load_3d(ringA + c * RPA + Cfg::ring_row_a(f * FR) * FWP, &p.tm[2], x0 - Cfg::XPAD, f * FR,
+                    b * C + c, bar);
+      tma_load_3d(st, &p.tm[1], x0 - Cfg::XPAD, f * FR, b * C, bar);
+      return;
+    }
 #pragma unroll
     for (int a = 0; a < Cfg::NARR; ++a) {
-      if (KIND != KX && vz && (a == 1 || a == 3)) continue;
+      if (!Cfg::ISX && vz && (a == 1 || a == 3)) continue;
       tma_load_3d(st + a * Cfg::ARRB, &p.tm[a], x0 - Cfg::XPAD, f * FR, b * C, bar);
     }
   };
@@ -244,10 +265,24 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     const real* rphi = reinterpret_cast<const real*>(st);
     const real* rvel = reinterpret_cast<const real*>(st + Cfg::ARRB);
     vreal A[C], Bf[C];
+    if constexpr (Cfg::DIRECT) {  // phi is in ring A already (TMA); the stage holds v only
+      const int ao = Cfg::ring_row_a(gy) * FWP + lx;
+#pragma unroll
+      for (int c = 0; c < C; ++c) A[c] = Bf[c] = vload<vreal>(ringA + c * RPA + ao);
+      if (inter) {
+#pragma unroll
+        for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * vload<vreal>(rphi + c * FR * RW + ro);
+        Th::project_field(Bf);
+      }
+      const int wb = Cfg::ring_row(gy) * FWP + lx;
+#pragma unroll
+      for (int c = 0; c < C; ++c) vstore(ringB + c * RP + wb, Bf[c]);
+      return;
+    }
 #pragma unroll
     for (int c = 0; c < C; ++c) A[c] = Bf[c] = vload<vreal>(rphi + c * FR * RW + ro);
     if (inter) {  // halo sites of every stage field are the frozen halo
-      if (KIND == KX) {
+      if (Cfg::ISX) {
 #pragma unroll
         for (int c = 0; c < C; ++c) Bf[c] = A[c] + p.hdt * vload<vreal>(rvel + c * FR * RW + ro);
         Th::project_field(Bf);
@@ -282,10 +317,10 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
         Th::project_field(Bf);
       }
     }
-    const int wo = Cfg::ring_row(gy) * FWP + lx;
+    const int wo = Cfg::ring_row(gy) * FWP + lx;  // not DIRECT: both rings have RING rows
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      vstore(ringA + c * RP + wo, A[c]);
+      vstore(ringA + c * RPA + wo, A[c]);
       if (KIND != KV) vstore(ringB + c * RP + wo, Bf[c]);
     }
   };
@@ -332,18 +367,21 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     if (!EDGE || (sc >= cs && sc < ce)) {
       const int gy0 = sc * FR + r0;
       // ring offsets of rows gy0-2 .. gy0+SPT+1 at the thread's column
-      int rw[SPT + 4];
+      int rw[SPT + 4], rwa[SPT + 4];  // ring B / ring A (the same unless DIRECT)
 #pragma unroll
-      for (int j = 0; j < SPT + 4; ++j) rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
+      for (int j = 0; j < SPT + 4; ++j) {
+        rw[j] = Cfg::ring_row(gy0 - HALO + j) * FWP + tx + HALO;
+        rwa[j] = Cfg::ring_row_a(gy0 - HALO + j) * FWP + tx + HALO;
+      }
       // tile accessor: component c, ring row slot j, x offset dx of the thread's first column;
       // with two columns per thread the odd offsets are recombined from the aligned pairs
-      auto tile = [&](const real* ring, const vreal (&colr)[C][SPT + 4], const int (&rwr)[SPT + 4],
-                      int c, int j, int dx) -> vreal {
+      auto tile = [&](const real* ring, const int rp, const vreal (&colr)[C][SPT + 4],
+                      const int (&rwr)[SPT + 4], int c, int j, int dx) -> vreal {
         if constexpr (VEC == 1) {
-          return dx == 0 ? colr[c][j] : vreal(ring[c * RP + rwr[j] + dx]);
+          return dx == 0 ? colr[c][j] : vreal(ring[c * rp + rwr[j] + dx]);
         } else {
           auto pr = [&](int dxe) -> vreal {
-            return dxe == 0 ? colr[c][j] : vload<vreal>(ring + c * RP + rwr[j] + dxe);
+            return dxe == 0 ? colr[c][j] : vload<vreal>(ring + c * rp + rwr[j] + dxe);
           };
           if (dx == 0 || dx == 2 || dx == -2) return pr(dx);
           if (dx == 1) return vreal(vhi(pr(0)), vlo(pr(2)));
@@ -367,13 +405,13 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       // Abelian Higgs: (12h)^2 DxDy A_c = D_y (D_x A_c) down the thread's column: one eq. (1)
       // numerator per ring row (4 loads) shared by the SPT sites, instead of 16 loads per site
       [[maybe_unused]] vreal xy[SPT][2];
-      [[maybe_unused]] auto mixed = [&](const real* ring) {
+      [[maybe_unused]] auto mixed = [&](const real* ring, const int rp, const int (&rwr)[SPT + 4]) {
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
           vreal dxr[SPT + 4];
 #pragma unroll
           for (int j = 0; j < SPT + 4; ++j) {
-            const real* q = ring + (2 + cc) * RP + rw[j];
+            const real* q = ring + (2 + cc) * rp + rwr[j];
             dxr[j] = d1n<vreal>(vreal(q[-2]), vreal(q[-1]), vreal(q[1]), vreal(q[2]));
           }
 #pragma unroll
@@ -383,17 +421,17 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
       };
       constexpr bool AHXY = THEORY == kAH && VEC == 1;
       // ---- ring A (X: phi -> a1, e, q    Y: phi3 -> a3)
-      if constexpr (AHXY) mixed(ringA);
+      if constexpr (AHXY) mixed(ringA, RPA, rwa);
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringA + c * RP + rw[j]);
+        for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringA + c * RPA + rwa[j]);
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         if (act[k]) {
           const int gy = gy0 + k;
-          auto TA = [&](int c, int dy, int dx) -> vreal { return tile(ringA, col, rw, c, k + dy + 2, dx); };
-          if (KIND == KX || KIND == KV) {
+          auto TA = [&](int c, int dy, int dx) -> vreal { return tile(ringA, RPA, col, rwa, c, k + dy + 2, dx); };
+          if (Cfg::ISX || KIND == KV) {
             vreal e, q;
             if (EDGE && (xedge || gy < 2 * HALO || gy >= Ny - 2 * HALO)) {
               if constexpr (AHXY) Th::accel_xy(TA, p, Bz, xy[k][0], xy[k][1], aA[k]);
@@ -406,7 +444,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
             }
             s0[k] = vsum(e);
             s1[k] = vsum(q);
-            if (KIND == KX) {
+            if (Cfg::ISX) {
 #pragma unroll
               for (int c = 0; c < C; ++c) vstore(o0 + c * p.plane + k * Nx, aA[k][c]);
             } else {  // second half kick, tangent projection, KE
@@ -439,16 +477,16 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
         for (int c = 0; c < C; ++c)
 #pragma unroll
           for (int j = 0; j < SPT + 4; ++j) col[c][j] = vload<vreal>(ringB + c * RP + rw[j]);
-        if constexpr (AHXY) mixed(ringB);
+        if constexpr (AHXY) mixed(ringB, RP, rw);
       }
 #pragma unroll
       for (int k = 0; k < SPT; ++k) {
         if (KIND != KV && act[k]) {
-          auto TB = [&](int c, int dy, int dx) -> vreal { return tile(ringB, col, rw, c, k + dy + 2, dx); };
+          auto TB = [&](int c, int dy, int dx) -> vreal { return tile(ringB, RP, col, rw, c, k + dy + 2, dx); };
           vreal aB[C];
           if constexpr (AHXY) Th::accel_xy(TB, p, Bz, xy[k][0], xy[k][1], aB);
           else Th::accel(TB, p, Bz, aB);
-          if (KIND == KX) {
+          if (Cfg::ISX) {
 #pragma unroll
             for (int c = 0; c < C; ++c) vstore(o1 + c * p.plane + k * Nx, aB[c]);
           } else {
@@ -478,7 +516,7 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
         // VEC == 2: one warp holds the whole 64-site row segment (pair sums = tree level 1)
         double* rr = red + (((f & 1) * 3) * FR + r0 + k) * 2 + (VEC == 2 ? 0 : (tx >> 5));
         if (VEC == 2 && lane < NQ) rr[lane * FR * 2 + 1] = 0.0;
-        if (KIND == KX || KIND == KV) {
+        if (Cfg::ISX || KIND == KV) {
           const double t = warp_tree2(s0[k], s1[k], lane);
           if (lane < 2) rr[lane * FR * 2] = t;
           if (KIND == KV) {
