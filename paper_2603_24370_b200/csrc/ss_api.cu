@@ -1287,6 +1287,7 @@ const char* ss_schedule_name(const ss_solver* s) {
   if (!s) return "";
   if (s->res_cl > 0) return "resident-cluster";
   if (s->ktheory == kBS) return "per-stage tile kernels";
+  if (s->demag != 0.0) return "pointwise kernels + multigrid V-cycles";
   if (s->slabs > 1) return "two-kernel, row slabs";
   return s->integrator == SS_VERLET ? "one-kernel verlet" : "two-kernel";
 }
