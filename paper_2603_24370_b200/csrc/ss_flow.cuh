@@ -101,6 +101,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, in
       : "memory");
 }
 
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* tm, int x, int y, int z) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(tm), "r"(x),
+               "r"(y), "r"(z)
+               : "memory");
+}
+
 // Shape of the march, per kernel (measured on B200): 2 vertically adjacent
 // sites per thread, 14-row rings (chunks f-1, f, f+1 and two rows of f-2 are live, one barrier
 // per chunk), 3 CTAs per SM; two TMA stages in X and V, one in Y (so that the third CTA fits).
@@ -241,6 +247,17 @@ __global__ void __launch_bounds__(FlowCfg<THEORY, real, KIND>::THREADS,
     for (int a = 0; a < Cfg::NARR; ++a) {
       if (!Cfg::ISX && vz && (a == 1 || a == 3)) continue;
       tma_load_3d(st + a * Cfg::ARRB, &p.tm[a], x0 - Cfg::XPAD, f * FR, b * C, bar);
+    }
+    // Kernel Y has a single stage (17 % of its stall samples wait for it): the boxes of the chunk
+    // after this one are pulled into the L2 now, so that their TMA load, issued one chunk later,
+    // has the short latency.  Y alone 0.458 -> 0.444 ms, fp32 0.243 -> 0.230; no gain for X and V
+    // (two stages), and nothing at two chunks ahead.
+    if (KIND == KY && f + 1 <= f1) {
+#pragma unroll
+      for (int a = 0; a < Cfg::NARR; ++a) {
+        if (vz && (a == 1 || a == 3)) continue;
+        tma_prefetch_3d(&p.tm[a], x0 - Cfg::XPAD, (f + 1) * FR, b * C);
+      }
     }
   };
   if (tid == 0)
