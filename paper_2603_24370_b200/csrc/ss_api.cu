@@ -567,11 +567,12 @@ int choose_cps(int nstrips, int Ny, int batch, int slots) {
 }
 
 // Row-slab pipelining of the RK4 step (ss_create): one lattice, tall enough for SLABS slabs of at
-// least two segments each, and at least three waves of CTAs -- below that the split only costs
-// (cm 1024^2: 0.084 vs 0.079 ms; 256 lattices of 256^2 split by lattice: -0.3 %, not built).
-// With the tail of Y filled by X the best segment is shorter than choose_cps's: about four
-// waves of CTAs in all, not below 12 chunks (measured: cm 4096^2 fp64 flat over 22..38 chunks,
-// fp32 best at 24, Abelian Higgs 2048^2 best at 14..16).
+// least two segments each, and at least two waves of CTAs -- below that the split only costs
+// (cm 1024^2: 0.084 vs 0.074 ms, 1280^2: 0.107 vs 0.109; 256 lattices of 256^2 split by lattice:
+// -0.3 %, not built).  With the tail of Y filled by X the best segment is shorter than
+// choose_cps's: about four waves of CTAs in all, not below 8 chunks (measured: cm 4096^2 fp64
+// flat over 22..38 chunks, fp32 best at 24, Abelian Higgs 2048^2 best at 14..16, cm 1536^2 and
+// 1792^2 best at 8: 0.139 vs 0.146 and 0.178 vs 0.192 ms without slabs).
 constexpr int SLABS = 4;
 void plan_slabs(ss_solver* s, int user_cps, int slots) {
   s->slabs = 0;
@@ -582,10 +583,10 @@ void plan_slabs(ss_solver* s, int user_cps, int slots) {
   if (cps <= 0) {
     const int segs = (4 * slots + s->L.nseg - 1) / s->L.nseg;
     cps = (NC + segs - 1) / (segs > 0 ? segs : 1);
-    if (cps < 12) cps = 12;
+    if (cps < 8) cps = 8;
   }
   const int nsy = (NC + cps - 1) / cps;
-  if (nsy < 2 * SLABS || (long long)nsy * s->L.nseg < 3LL * slots) return;
+  if (nsy < 2 * SLABS || (long long)nsy * s->L.nseg < 2LL * slots) return;
   s->slabs = SLABS;
   s->cps[KX] = s->cps[KY] = cps;
 }
@@ -885,7 +886,8 @@ int ss_create(ss_solver** out, int theory, int Nx, int Ny, double h, const ss_pa
   }
   plan_slabs(s, p->chunks_per_segment, slots[KX] < slots[KY] ? slots[KX] : slots[KY]);
   // Without row slabs kernel X takes phi by TMA straight into its ring (ss_flow.cuh KXD: 4 CTAs
-  // per SM; 256 x 256^2 0.924 vs 0.940 ms, cm 1024^2 0.075 vs 0.078).  Inside the slab schedule
+  // per SM; 256 x 256^2 0.917 vs 0.936 ms, cm 512^2 ... 1536^2 and 4 ... 64 batched lattices 1 ... 8 %
+  // faster than KX).  Inside the slab schedule
   // its single TMA stage waits longer while Y streams (cm 4096^2 0.807 vs 0.793): KX there.
   s->xkind = (has_xd && s->slabs == 0 && s->integrator == SS_RK4) ? KXD : KX;
   for (int cur = 0; cur < 2; ++cur) {

@@ -64,7 +64,9 @@ def test_slab_schedule_is_bitwise_identical_and_matches_the_oracle(case):
 
 def test_slabs_are_not_used_where_they_do_not_pay():
     ss = _ss()
-    assert ss.solver_for(W.cm_multi(N=1024)).schedule() == "two-kernel"          # < 3 waves
+    assert ss.solver_for(W.cm_multi(N=1024)).schedule() == "two-kernel"          # < 2 waves
+    assert ss.solver_for(W.cm_quench(N=1280)).schedule() == "two-kernel"
+    assert ss.solver_for(W.cm_quench(N=1536)).schedule() == "two-kernel, row slabs"
     assert ss.solver_for(W.cm_sweep(batch=4, N=256)).schedule() == "two-kernel"   # batched
     assert ss.solver_for(W.cm_quench(N=2048), integrator=ss.VERLET).schedule() == "one-kernel verlet"
     assert ss.solver_for(W.cm_quench(N=4096)).schedule() == "two-kernel, row slabs"
