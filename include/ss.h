@@ -164,10 +164,11 @@ int ss_get_fields_host(ss_solver* s, void* fields_host, void* vel_host);
  * shared memory of one thread-block cluster per lattice, e.g. 64 x 64 ... 128 x 128) take all k
  * steps in ONE launch with the state resident in shared memory; fields, E, Q, KE and the arrest
  * log are bitwise identical to the general schedule.
- * Large single lattices (SS_RK4, at least two waves of CTAs and eight row segments: from about
- * 1536 x 1536 sites) have the step's two flow kernels split into four row
- * slabs each, joined in the graph by the data dependencies only, so that the second kernel
- * starts on the rows the first has finished; again bitwise identical (SS_FLAG_NO_SLABS). */
+ * Large lattices (SS_RK4, at least two waves of CTAs and eight row segments per lattice: from
+ * about 1536 x 1536 sites, or a few batched 512 x 512 ones) have the step's two flow kernels
+ * split into four row slabs each, joined in the graph by the data dependencies only, so that
+ * the second kernel starts on the rows the first has finished; again bitwise identical
+ * (SS_FLAG_NO_SLABS). */
 int ss_step(ss_solver* s, int64_t k);
 
 /* Scalar read-outs: synchronise the stream, then fill HOST arrays of length batch.

@@ -566,27 +566,31 @@ int choose_cps(int nstrips, int Ny, int batch, int slots) {
   return best_cps;
 }
 
-// Row-slab pipelining of the RK4 step (ss_create): one lattice, tall enough for SLABS slabs of at
+// Row-slab pipelining of the RK4 step (ss_create): lattices tall enough for SLABS slabs of at
 // least two segments each, and at least two waves of CTAs -- below that the split only costs
-// (cm 1024^2: 0.084 vs 0.074 ms, 1280^2: 0.107 vs 0.109; 256 lattices of 256^2 split by lattice:
-// -0.3 %, not built).  With the tail of Y filled by X the best segment is shorter than
+// (cm 1024^2: 0.084 vs 0.074 ms, 1280^2: 0.107 vs 0.109).  Batched lattices are split the same
+// way, every slab launch covering its rows of all lattices (4 x 1024^2: 0.246 -> 0.227 ms, 16 x
+// 512^2: 0.283 -> 0.237, 2 x 2048^2: 0.459 -> 0.406); many small lattices do not qualify (256 x
+// 256^2: two segments of four waves' length per lattice; split by lattice instead: -0.3 %, not
+// built).  With the tail of Y filled by X the best segment is shorter than
 // choose_cps's: about four waves of CTAs in all, not below 8 chunks (measured: cm 4096^2 fp64
 // flat over 22..38 chunks, fp32 best at 24, Abelian Higgs 2048^2 best at 14..16, cm 1536^2 and
 // 1792^2 best at 8: 0.139 vs 0.146 and 0.178 vs 0.192 ms without slabs).
 constexpr int SLABS = 4;
 void plan_slabs(ss_solver* s, int user_cps, int slots) {
   s->slabs = 0;
-  if (s->integrator != SS_RK4 || s->ktheory == kBS || s->demag != 0.0 || s->batch != 1) return;
+  if (s->integrator != SS_RK4 || s->ktheory == kBS || s->demag != 0.0) return;
+  const int min_nsy = 2 * SLABS;
   if (s->flags & SS_FLAG_NO_SLABS) return;
   const int NC = (s->Ny + FR - 1) / FR;
   int cps = user_cps;
   if (cps <= 0) {
-    const int segs = (4 * slots + s->L.nseg - 1) / s->L.nseg;
+    const int segs = (4 * slots + s->L.nseg * s->batch - 1) / (s->L.nseg * s->batch);
     cps = (NC + segs - 1) / (segs > 0 ? segs : 1);
     if (cps < 8) cps = 8;
   }
   const int nsy = (NC + cps - 1) / cps;
-  if (nsy < 2 * SLABS || (long long)nsy * s->L.nseg < 2LL * slots) return;
+  if (nsy < min_nsy || (long long)nsy * s->L.nseg * s->batch < 2LL * slots) return;
   s->slabs = SLABS;
   s->cps[KX] = s->cps[KY] = cps;
 }

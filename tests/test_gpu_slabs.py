@@ -28,14 +28,16 @@ def _cases():
     yield "cm", W.cm_quench(N=644), False, True, 12
     yield "cm_f32", W.cm_quench(N=900), True, False, 12
     yield "ah", W.ah_vortices(N=516, h=0.1, lam=2.0, count=2, min_sep=2.0), False, False, 8
+    yield "cm_batched", W.cm_sweep(batch=3, N=324), False, False, 10
 
 
-@pytest.mark.parametrize("case", ["cm", "cm_f32", "ah"])
+@pytest.mark.parametrize("case", ["cm", "cm_f32", "ah", "cm_batched"])
 def test_slab_schedule_is_bitwise_identical_and_matches_the_oracle(case):
     ss = _ss()
     name, w, f32, uphill, steps = next(c for c in _cases() if c[0] == case)
     td = torch.float32 if f32 else torch.float64
-    m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=w.B, K=w.K, lam=w.lam)
+    B0 = w.B if w.B_batch is None else float(w.B_batch[0])
+    m = oracle.model(w.theory, w.Nx, w.Ny, w.h, kappa=w.kappa, B=B0, K=w.K, lam=w.lam)
     vel = (-0.06 * oracle.accel(m, w.fields[0]))[None] if uphill else None
     outs = {}
     for flags in (ss.FLAG_NO_SLABS, 0, ss.FLAG_NO_GRAPH):
@@ -67,7 +69,8 @@ def test_slabs_are_not_used_where_they_do_not_pay():
     assert ss.solver_for(W.cm_multi(N=1024)).schedule() == "two-kernel"          # < 2 waves
     assert ss.solver_for(W.cm_quench(N=1280)).schedule() == "two-kernel"
     assert ss.solver_for(W.cm_quench(N=1536)).schedule() == "two-kernel, row slabs"
-    assert ss.solver_for(W.cm_sweep(batch=4, N=256)).schedule() == "two-kernel"   # batched
+    assert ss.solver_for(W.cm_sweep(batch=4, N=256)).schedule() == "two-kernel"   # small lattices
+    assert ss.solver_for(W.cm_sweep(batch=4, N=1024)).schedule() == "two-kernel, row slabs"
     assert ss.solver_for(W.cm_quench(N=2048), integrator=ss.VERLET).schedule() == "one-kernel verlet"
     assert ss.solver_for(W.cm_quench(N=4096)).schedule() == "two-kernel, row slabs"
 
