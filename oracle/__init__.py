@@ -204,7 +204,10 @@ class Flow:
 
     def __del__(self):
         if getattr(self, "_h", None):
-            lib().orc_flow_destroy(self._h)
+            try:
+                lib().orc_flow_destroy(self._h)
+            except TypeError:      # interpreter shutdown: the module globals are already gone
+                pass
             self._h = None
 
     def set_fields(self, phi, vel=None):
