@@ -116,3 +116,36 @@ def test_profile_step_under_the_slab_schedule_advances_like_step():
     fb, vb = b.get_fields()
     assert torch.equal(fa, fb) and torch.equal(va, vb)
     assert a.energy() == b.energy() and a.status()["steps"] == b.status()["steps"] == 9
+
+
+@pytest.mark.parametrize("shape", [(6000, 1000, 1, "cm"), (66, 20000, 1, "cm"), (2002, 702, 3, "cm"),
+                                   (518, 3000, 2, "ah")])
+def test_slabs_on_ragged_non_square_and_batched_shapes(shape):
+    # the default segment length and slab split on shapes whose sizes divide nothing evenly: wide,
+    # tall and narrow, batched; random fields; bitwise against the unsplit step
+    ss = _ss()
+    Nx, Ny, batch, th = shape
+    rng = np.random.default_rng(Nx + Ny)
+    theory = W.AH if th == "ah" else W.CM
+    f = rng.standard_normal((batch, 4 if th == "ah" else 3, Ny, Nx))
+    if th == "cm":
+        f /= np.sqrt((f * f).sum(1, keepdims=True))
+        f[:, :, ~W.interior_mask(Nx, Ny)] = np.array([0.0, 0.0, 1.0])[None, :, None]
+    else:
+        f *= 0.3
+        f[:, 0] += 1.0
+    h = 0.1 if th == "ah" else 0.2
+    w = W.Workload("shape", theory, Nx, Ny, h, 0.5 * h, kappa=1.0, B=0.6, K=0.1, lam=1.5, batch=batch,
+                   fields=f)
+    outs = []
+    for flags in (ss.FLAG_NO_SLABS, 0):
+        s = ss.solver_for(w, flags=flags)
+        s.set_fields(_dev(w.fields))
+        s.step(11)
+        fo, vo = s.get_fields()
+        outs.append((fo, vo, s.energy(), s.charge(), s.kinetic(), [s.arrests(k) for k in range(batch)],
+                     s.schedule()))
+        del s
+    assert outs[0][6] == "two-kernel" and outs[1][6] == "two-kernel, row slabs"
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    assert outs[0][2:6] == outs[1][2:6]
