@@ -683,6 +683,8 @@ int build_graph(ss_solver* s, std::vector<KernelNode>& nodes, cudaGraphExec_t* e
   cudaError_t e = cudaGraphInstantiate(exec, g, 0);
   cudaGraphDestroy(g);
   if (!cuda_ok(e, "cudaGraphInstantiate")) return SS_ERR_CUDA;
+  // upload now: otherwise the first launch of each graph pays for it inside the caller's timing
+  if (!cuda_ok(cudaGraphUpload(*exec, s->stream), "cudaGraphUpload")) return SS_ERR_CUDA;
   return SS_OK;
 }
 
