@@ -34,8 +34,9 @@
  *   Memory    every pointer named *_dev is DEVICE memory owned by the caller; every pointer
  *             named *_host is HOST memory owned by the caller.  The library allocates no
  *             device memory: all of its state lives in the caller's `workspace`
- *             (ss_workspace_bytes), which must outlive the handle.  The caller also owns the
- *             CUDA stream; all work is enqueued on it.
+ *             (ss_workspace_bytes), which must outlive the handle (the only device memory of
+ *             its own is the static 256 KiB scratch array of ss_render_noalloc).  The caller
+ *             also owns the CUDA stream; all work is enqueued on it.
  *   Errors    every call returns an SS_* status; nothing throws or aborts across the ABI.
  *   Threads   a handle is not thread-safe; distinct handles are independent.
  *   No CPU fallback exists: without a CUDA device ss_create returns SS_ERR_CUDA.
